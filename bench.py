@@ -1,0 +1,401 @@
+#!/usr/bin/env python
+"""bench.py -- FPN RoIAlign fwd+bwd throughput on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (level assignment + forward gather + backward scatter,
+incl. zero-fill) over one synthetic batch of BASELINE.json configs[1] (Faster R-CNN R-50-FPN box
+head, training: batch 2, 4 levels, C=256 fp32, 1024 RoIs, 7x7, sampling_ratio 2), through the C ABI.
+
+  python bench.py --gpus N --steps K --warmup W            our arm (one rank per GPU; no collective:
+                                                           the path shards by image -> weak scaling)
+  python bench.py --impl reference ...                     the CPU oracle on the host cores
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 6 for every field.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "RoIAlign fwd+bwd RoIs/sec (C=256, 7x7, FPN)"
+UNIT = "RoIs/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based)")
+    ap.add_argument("--layout", default="cl", choices=["cl", "nchw"])
+    ap.add_argument("--deterministic", action="store_true", help="time the RAF_DETERMINISTIC backward")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--graph", action="store_true", help="replay each step from a CUDA graph")
+    return ap.parse_args()
+
+
+def peaks():
+    """Measured peak (driver-written MEASURED_PEAKS.json) or the profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+class OracleLeg:
+    """The oracle as it stands, timed on the host cores on a bounded sample of the workload: all
+    channels, the first `n` RoIs of each image of the config (fwd, + bwd when the config has one).
+    `n` is chosen from a short probe so that one pass takes at most about `budget_s` seconds."""
+
+    def __init__(self, cfg_index):
+        from oracle import raf_ref as R
+        from paper_1906_07155_b200 import inputs
+        self.R, self.index = R, cfg_index
+        self.cfg = cfg = inputs.CONFIGS[cfg_index]
+        self.wl = inputs.make_workload(cfg_index)
+        self.feats64 = [f.astype(np.float64) for f in self.wl.feats]
+        self.gout64 = self.wl.grad_out.astype(np.float64)
+        self.sel = self._pick(cfg.per_img)
+
+    def _pick(self, n_per_img):
+        c = self.cfg
+        return np.concatenate([np.arange(i * c.per_img, i * c.per_img + n_per_img) for i in range(c.n_img)])
+
+    def run(self, sel=None):
+        c, R = self.cfg, self.R
+        sel = self.sel if sel is None else sel
+        t0 = time.perf_counter()
+        R.forward(self.feats64, c.scales, self.wl.rois[sel], c.out_size, c.sampling_ratio, c.aligned, c.finest_scale)
+        if c.backward:
+            R.backward(c.level_shapes, c.scales, self.gout64[sel], self.wl.rois[sel], c.out_size,
+                       c.sampling_ratio, c.aligned, c.finest_scale, want_abs_sum=False)
+        return time.perf_counter() - t0
+
+    def calibrate(self, budget_s):
+        c = self.cfg
+        probe_n = min(8, c.per_img)
+        t_probe = self.run(self._pick(probe_n))
+        t_fixed = self.run(self._pick(1))     # zero-fill of the double pyramid etc.
+        per_roi = max((t_probe - t_fixed) / max(c.n_img * (probe_n - 1), 1), 1e-7)
+        n = int(min(c.per_img, max(1, (budget_s - t_fixed) / per_roi / c.n_img)))
+        self.sel = self._pick(n)
+        return n
+
+    def describe(self, t, value):
+        c = self.cfg
+        n = len(self.sel) // c.n_img
+        return {"value": value, "unit": UNIT, "cores": self.R.num_threads(), "kind": "oracle",
+                "sample": f"config {self.index}: first {n} RoIs of each of {c.n_img} images ({len(self.sel)} of {c.K} "
+                          f"RoIs), all {c.channels} channels, fwd{'+bwd' if c.backward else ''}, spec mode, OpenMP; "
+                          f"{t:.2f} s per pass"}
+
+
+def cpu_baseline(cfg_index, budget_s=20.0):
+    leg = OracleLeg(cfg_index)
+    leg.calibrate(budget_s)
+    t = min(leg.run() for _ in range(3 if budget_s < 5 else 1))
+    return leg.describe(t, len(leg.sel) / t)
+
+
+def run_reference(args):
+    """--impl reference: the oracle (kind 'oracle') on the host cores; rank 0 only.  Each step is one
+    oracle pass over a bounded RoI sample sized so that steps+warmup end within about 150 s."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import build as ref_build
+    ref_build.build()
+    leg = OracleLeg(args.config)
+    cfg = leg.cfg
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    leg.calibrate(150.0 / (steps + warm))
+    for _ in range(warm):
+        leg.run()
+    times = [leg.run() for _ in range(steps)]
+    t = sum(times) / len(times)
+    value = len(leg.sel) / t
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": warm, "ms_per_step": 1e3 * t,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {cfg.name}",
+                                            "note": "each step = the oracle on a bounded RoI sample of the workload"},
+            "cpu_baseline": leg.describe(t, value),
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1906_07155_b200 import binding as B
+    from paper_1906_07155_b200 import build as raf_build
+    from paper_1906_07155_b200 import inputs, roofline
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py (our arm) needs a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if rank == 0:
+        raf_build.build()
+    if world > 1:
+        dist.barrier()
+    B.lib()
+
+    cfg = inputs.CONFIGS[args.config]
+    wl = inputs.make_workload(args.config)
+    tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[cfg.dtype]
+    esz = 4 if cfg.dtype == "f32" else 2
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    PH, PW = cfg.out_size
+    g, aligned, fs = cfg.sampling_ratio, cfg.aligned, cfg.finest_scale
+    flags = B.RAF_DETERMINISTIC if args.deterministic else 0
+
+    def lay(t):   # logical NCHW tensor -> requested physical layout
+        return t.contiguous() if args.layout == "nchw" else t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
+
+    pyr_bytes = sum(int(np.prod(s)) for s in cfg.level_shapes)
+    ws_set = pyr_bytes * esz + pyr_bytes * 4 * cfg.backward + K * C * PH * PW * esz * (1 + cfg.backward)
+    l2 = torch.cuda.get_device_properties(local_rank).L2_cache_size
+    R = int(max(4, -(-2 * l2 // ws_set)))
+    base_feats = [torch.from_numpy(f).to(tdt) for f in wl.feats]
+    feats = [[lay(f.cuda()) for f in base_feats] for _ in range(R)]
+    rois = torch.from_numpy(wl.rois).cuda()
+    outs = [lay(torch.empty((K, C, PH, PW), dtype=tdt, device="cuda")) for _ in range(R)]
+    gouts = [lay(torch.from_numpy(wl.grad_out).to(tdt).cuda()) for _ in range(R)] if cfg.backward else None
+    grads = [[lay(torch.empty(s, dtype=torch.float32, device="cuda")) for s in cfg.level_shapes]
+             for _ in range(R)] if cfg.backward else None
+    ws = torch.empty(B.roi_align_fpn_workspace_bytes(K, L, PH, PW, g, flags), dtype=torch.uint8, device="cuda")
+    fdesc = [B.make_levels(f, cfg.scales) for f in feats]
+    gdesc = [B.make_levels(gr, cfg.scales) for gr in grads] if cfg.backward else None
+    stream = torch.cuda.current_stream()
+
+    def fwd(j):
+        B.roi_align_fpn_forward(feats[j], cfg.scales, rois, outs[j], g, aligned, fs, ws, stream, fdesc[j])
+
+    def bwd(j):
+        B.roi_align_fpn_backward(grads[j], cfg.scales, gouts[j], rois, g, aligned, fs, flags, ws, stream, gdesc[j])
+
+    graphs = None
+    if args.graph:
+        graphs = []
+        for j in range(R):
+            fwd(j)
+            if cfg.backward:
+                bwd(j)
+        torch.cuda.synchronize()
+        for j in range(R):
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr):
+                s = torch.cuda.current_stream()
+                B.roi_align_fpn_forward(feats[j], cfg.scales, rois, outs[j], g, aligned, fs, ws, s, fdesc[j])
+                if cfg.backward:
+                    B.roi_align_fpn_backward(grads[j], cfg.scales, gouts[j], rois, g, aligned, fs, flags, ws, s, gdesc[j])
+            graphs.append(gr)
+
+    for i in range(args.warmup):
+        j = i % R
+        if graphs:
+            graphs[j].replay()
+        else:
+            fwd(j)
+            if cfg.backward:
+                bwd(j)
+    torch.cuda.synchronize()
+
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = B.launch_count()
+    for i in range(args.steps):
+        j = (args.warmup + i) % R
+        ev[i][0].record(stream)
+        if graphs:
+            graphs[j].replay()
+            ev[i][1].record(stream)
+        else:
+            fwd(j)
+            ev[i][1].record(stream)
+            if cfg.backward:
+                bwd(j)
+        ev[i][2].record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    launches = B.launch_count() - launches0
+    if graphs:   # replayed launches are not seen by the library's counter: count per captured step
+        launches = args.steps * (1 + (1 + L) * cfg.backward)
+    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    clocks = sampler.stop() if rank == 0 else None
+    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
+    bwd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev])) if cfg.backward and not graphs else None
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline (algorithmic bytes / CUDA-event duration of the dominant call) ----
+    fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, g, aligned, fs)
+    ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz)
+    peak, peak_src = peaks()
+    traffic = {}
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(f"config{args.config}", {})
+    legs = {"fwd": (ab["fwd"], fwd_ms)}
+    if bwd_ms is not None:
+        legs["bwd"] = (ab["bwd"], bwd_ms)
+    dom = max(legs, key=lambda k: legs[k][1])
+
+    def roof(name):
+        by, ms = legs[name]
+        ach = by / (ms * 1e-3) / 1e9
+        return {"bound": "hbm", "kernel": name, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": traffic.get(name), "algorithmic_bytes": by, "ms": ms, "peak_source": peak_src}
+
+    step_ms = total_ms / args.steps
+    step_bytes = ab["fwd"] + (ab["bwd"] if cfg.backward else 0)
+    line = {"metric": METRIC, "value": world * K / (step_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {cfg.name}", "K": K, "C": C,
+                       "out_size": [PH, PW], "levels": L, "layout": args.layout, "parallelism": f"replicas x{world} (shard by image, no collective)",
+                       "l2_protocol": f"inputs rotate over {R} independent copies ({R * ws_set / 1e6:.0f} MB >> L2 {l2 / 1e6:.0f} MB)",
+                       "backward": ("deterministic" if args.deterministic else "atomic") if cfg.backward else "none",
+                       "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
+            "roofline": roof(dom),
+            "roofline_all": {k: roof(k) for k in legs} | {"step": {"achieved": step_bytes / (step_ms * 1e-3) / 1e9,
+                                                                  "frac": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
+                                                                  "algorithmic_bytes": step_bytes, "ms": step_ms}},
+            "clocks": clocks, "gpu_launches": int(launches)}
+
+    # ---- e2e: HOST buffers through the C ABI, copies inside the timed region ----
+    if not args.no_e2e:
+        hf = [lay(f).pin_memory() if args.layout == "nchw" else f.permute(0, 2, 3, 1).contiguous().pin_memory().permute(0, 3, 1, 2)
+              for f in base_feats]
+        hrois = torch.from_numpy(wl.rois).pin_memory()
+
+        def hbuf(shape, dt):
+            n, c, h, w = shape
+            if args.layout == "nchw":
+                return torch.empty(shape, dtype=dt).pin_memory()
+            return torch.empty((n, h, w, c), dtype=dt).pin_memory().permute(0, 3, 1, 2)
+        hout = hbuf((K, C, PH, PW), tdt)
+        arena = torch.empty(B.roi_align_fpn_host_arena_bytes(hf, cfg.scales, tdt, K, PH, PW, g, flags),
+                            dtype=torch.uint8, device="cuda")
+        h2d = sum(f.numel() for f in hf) * esz + K * 20
+        d2h = K * C * PH * PW * esz
+        if cfg.backward:
+            hgout = hbuf((K, C, PH, PW), tdt)
+            hgout.copy_(torch.from_numpy(wl.grad_out).to(tdt))
+            hgrads = [hbuf(s, torch.float32) for s in cfg.level_shapes]
+            h2d += K * C * PH * PW * esz + K * 20
+            d2h += pyr_bytes * 4
+
+        def e2e_step():
+            B.roi_align_fpn_forward_host(hf, cfg.scales, hrois, hout, g, aligned, fs, arena, stream)
+            if cfg.backward:
+                B.roi_align_fpn_backward_host(hgrads, cfg.scales, hgout, hrois, g, aligned, fs, flags, arena, stream)
+        n_e2e = max(1, min(args.steps, 5))
+        e2e_step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n_e2e):
+            e2e_step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / n_e2e
+        line["e2e"] = {"value": world * K / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                       "d2h_bytes_per_step": int(d2h), "ms_per_step": ms, "steps": n_e2e,
+                       "note": "roi_align_fpn_{forward,backward}_host: pinned host buffers, copies in the timed region"}
+        del arena
+
+    if not args.no_cpu_baseline and world == 1:
+        from oracle import build as ref_build
+        ref_build.build()
+        line["cpu_baseline"] = cpu_baseline(args.config)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

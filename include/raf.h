@@ -1,0 +1,127 @@
+/* raf.h -- C ABI of libraf.so: B200-native multi-level (FPN) RoIAlign forward + backward.
+ *
+ * The operation is the RoIExtractor of a two-stage detector ("extracts RoI-wise features from a
+ * single or multiple feature maps with RoIPooling-like operators ... from the corresponding level
+ * of feature pyramids ... SingleRoIExtractor", section 3.1), run on the GPU as
+ * the paper claims for "all basic bbox and mask operations".  The paper gives no
+ * formula; the arithmetic is BASELINE.json `north_star` + the public RoIAlign definition (Mask
+ * R-CNN) as fixed in SURVEY.md section 8(c) C1-C5 and DESIGN.md section 3.
+ *
+ * General conventions
+ *  - Every pointer is a DEVICE pointer unless the parameter comment says HOST.
+ *  - The caller owns every buffer, including the workspace.  The library keeps no global state,
+ *    never allocates, never synchronises, never copies device->host (the *_host entry points below
+ *    are the stated exception: they copy between the caller's host buffers and the caller's
+ *    device arena).  All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the
+ *    legacy default stream).  Calls are CUDA-graph capturable.
+ *  - Return value: RAF_OK or a negative raf_status, decided on the host before any launch; no
+ *    exception crosses the ABI.  Launch failures are reported as RAF_ERR_CUDA.
+ *  - rois: float32 [K,5] row-major, row = (batch_idx, x1, y1, x2, y2) in image pixels.  A RoI whose
+ *    batch_idx is not an integer in [0,N) yields an all-zero output row and no gradient.
+ *    Non-finite coordinates are memory-safe but unspecified in value.
+ *  - K == 0 returns RAF_OK without launching (backward still zero-fills in overwrite mode).
+ */
+#ifndef RAF_H_
+#define RAF_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  RAF_OK = 0,
+  RAF_ERR_NULL = -1,        /* a required pointer is NULL                                        */
+  RAF_ERR_SHAPE = -2,       /* L not in [1,8], K < 0, out_h/out_w not in [1,32], sampling_ratio < 0
+                               or > 16, n/c mismatch across levels, non-positive dimension        */
+  RAF_ERR_DTYPE = -3,       /* unknown raf_dtype                                                  */
+  RAF_ERR_STRIDE = -4,      /* zero / negative stride, or a stride layout that aliases            */
+  RAF_ERR_UNSUPPORTED = -5, /* valid request this version does not implement                      */
+  RAF_ERR_WORKSPACE = -6,   /* ws_bytes smaller than roi_align_fpn_workspace_bytes()              */
+  RAF_ERR_CUDA = -7         /* a CUDA runtime call / launch failed                                */
+} raf_status;
+
+typedef enum { RAF_F32 = 0, RAF_F16 = 1, RAF_BF16 = 2 } raf_dtype;
+
+/* One FPN level.  The array of L descriptors lives in HOST memory and is read at call time. */
+typedef struct {
+  void* data;             /* DEVICE pointer: features (read-only) or gradients (written)           */
+  int32_t n, c, h, w;     /* logical shape [N,C,H,W]; n and c identical across levels              */
+  int64_t sn, sc, sh, sw; /* strides in ELEMENTS: NCHW and channels-last are both expressible      */
+  float spatial_scale;    /* 1/stride of the level (0.25, 0.125, ...)                              */
+} raf_level;
+
+/* Backward flags (bitmask). */
+enum {
+  RAF_ACCUMULATE = 1,     /* add into the existing gradient pyramid instead of overwriting it      */
+  RAF_DETERMINISTIC = 2   /* bit-reproducible run to run (pull / sorted-segment variant, K3d)      */
+};
+
+/* Bytes of device workspace the calls below need for these arguments (never 0; 256-aligned). */
+size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,
+                                     int flags);
+
+/* Level assignment + per-level histogram + stable bucketing (north_star).
+ *   level_k = #{ j in [1,L-1] : t_k >= 2^j },  t_k = sqrt((x2-x1)*(y2-y1)) / finest_scale + 1e-6f,
+ *   every operation an individually rounded fp32 IEEE operation (== clamp(floor(log2 t),0,L-1)).
+ *   counts[l] = #{k : level_k = l};  perm = RoI indices grouped by level, ascending k inside a
+ *   level (stable).  levels[K], counts[L], perm[K] are int32 DEVICE buffers; any of the three may
+ *   be NULL if not wanted. */
+int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
+                          int32_t* counts, int32_t* perm, void* ws, size_t ws_bytes, void* stream);
+
+/* Forward:
+ *   out[k,c,ph,pw] = (1/count) * sum_{iy<gh, ix<gw} bilinear(F_{level_k}[b_k,c], y(ph,iy), x(pw,ix))
+ * with fp32 sample coordinates in the canonical operation order, fp32 accumulation.
+ *   feats        HOST array of L descriptors (device data pointers), dtype = `dtype`
+ *   out          DEVICE, dtype = `dtype`, logical [K,C,out_h,out_w] addressed through
+ *                out_strides (HOST array of 4 element strides); row k = RoI k (original order)
+ *   sampling_ratio  > 0: fixed grid; 0: adaptive gh = ceil(roi_h/out_h), gw = ceil(roi_w/out_w)
+ *   aligned      != 0: half-pixel shift, no minimum box size; 0: legacy (no shift, size >= 1)   */
+int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                          int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
+                          void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,
+                          void* stream);
+
+/* Backward: exact transpose of the forward.
+ *   grad_feats   HOST array of L descriptors; data = fp32 DEVICE gradient pyramid, same logical
+ *                shapes as the features.  Overwritten (every element written: zero or sum) unless
+ *                RAF_ACCUMULATE.
+ *   grad_out     DEVICE, dtype = gout_dtype, logical [K,C,out_h,out_w] through gout_strides (HOST)
+ *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC                                              */
+int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
+                           const void* grad_out, const int64_t* gout_strides, const float* rois,
+                           int K, int out_h, int out_w, int sampling_ratio, int aligned,
+                           float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream);
+
+/* End-to-end variants with HOST buffers (used for the e2e benchmark line): every `data` pointer in
+ * the descriptors, `rois`, `out` / `grad_out` are HOST pointers (pinned for full copy speed) and
+ * must be contiguous in the order the strides describe (each level / tensor occupies exactly
+ * n*c*h*w resp. K*C*out_h*out_w elements).  The call copies the inputs into `arena` (DEVICE,
+ * caller-owned, at least roi_align_fpn_host_arena_bytes()), runs the device path, and copies the
+ * result back, all on `stream`; it does not synchronise. */
+size_t roi_align_fpn_host_arena_bytes(const raf_level* levels, int L, raf_dtype dtype, int K,
+                                      int out_h, int out_w, int sampling_ratio, int flags);
+int roi_align_fpn_forward_host(const raf_level* feats_host, int L, raf_dtype dtype,
+                               const float* rois_host, int K, int out_h, int out_w,
+                               int sampling_ratio, int aligned, float finest_scale, void* out_host,
+                               const int64_t* out_strides, void* arena, size_t arena_bytes,
+                               void* stream);
+int roi_align_fpn_backward_host(const raf_level* grad_feats_host, int L, raf_dtype gout_dtype,
+                                const void* grad_out_host, const int64_t* gout_strides,
+                                const float* rois_host, int K, int out_h, int out_w,
+                                int sampling_ratio, int aligned, float finest_scale, int flags,
+                                void* arena, size_t arena_bytes, void* stream);
+
+/* Static description of a status code. */
+const char* roi_align_fpn_strerror(int status);
+
+/* Number of kernels the library has launched in this process (monotonic; for bench accounting). */
+uint64_t roi_align_fpn_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RAF_H_ */

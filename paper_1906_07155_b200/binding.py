@@ -1,0 +1,190 @@
+"""Thin ctypes binding of libraf.so (include/raf.h).  Argument marshalling only: every step of the
+path (level assignment, bucketing, forward gather, backward scatter, zero-fill) runs in the CUDA
+kernels behind the C ABI.  PyTorch is used for device memory and the current stream, nothing else.
+
+There is NO fallback: if libraf.so is missing or a call returns a negative status, this raises.
+Function names equal the C entry points.
+"""
+import ctypes
+import os
+from typing import List, Optional, Sequence, Tuple
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libraf.so")
+
+RAF_F32, RAF_F16, RAF_BF16 = 0, 1, 2
+RAF_ACCUMULATE, RAF_DETERMINISTIC = 1, 2
+_DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_BF16}
+
+EXPORTS = [
+    "roi_align_fpn_workspace_bytes", "roi_fpn_assign_levels", "roi_align_fpn_forward",
+    "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
+    "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
+]
+
+
+class RafLevel(ctypes.Structure):
+    _fields_ = [("data", ctypes.c_void_p), ("n", ctypes.c_int32), ("c", ctypes.c_int32),
+                ("h", ctypes.c_int32), ("w", ctypes.c_int32), ("sn", ctypes.c_int64),
+                ("sc", ctypes.c_int64), ("sh", ctypes.c_int64), ("sw", ctypes.c_int64),
+                ("spatial_scale", ctypes.c_float)]
+
+
+class RafError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: raf_status {status} ({strerror(status)})")
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libraf.so; fails loudly if the CUDA library has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} not found: build it with "
+                               "`python -m paper_1906_07155_b200.build` (no CPU fallback exists)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.roi_align_fpn_workspace_bytes.restype = ctypes.c_size_t
+        L.roi_align_fpn_workspace_bytes.argtypes = [ctypes.c_int] * 6
+        L.roi_align_fpn_host_arena_bytes.restype = ctypes.c_size_t
+        L.roi_align_fpn_host_arena_bytes.argtypes = [ctypes.c_void_p] + [ctypes.c_int] * 7
+        L.roi_fpn_assign_levels.restype = ctypes.c_int
+        L.roi_fpn_assign_levels.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_float,
+                                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                            ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        fwd_args = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_int,
+                    ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_float,
+                    ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p]
+        bwd_args = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                    ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                    ctypes.c_int, ctypes.c_float, ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t,
+                    ctypes.c_void_p]
+        for name, args in (("roi_align_fpn_forward", fwd_args), ("roi_align_fpn_forward_host", fwd_args),
+                           ("roi_align_fpn_backward", bwd_args), ("roi_align_fpn_backward_host", bwd_args)):
+            getattr(L, name).restype = ctypes.c_int
+            getattr(L, name).argtypes = args
+        L.roi_align_fpn_strerror.restype = ctypes.c_char_p
+        L.roi_align_fpn_strerror.argtypes = [ctypes.c_int]
+        L.roi_align_fpn_launch_count.restype = ctypes.c_uint64
+        _lib = L
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return lib().roi_align_fpn_strerror(int(status)).decode()
+
+
+def launch_count() -> int:
+    return int(lib().roi_align_fpn_launch_count())
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> ctypes.c_void_p:
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _ptr(t: Optional[torch.Tensor]) -> ctypes.c_void_p:
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def make_levels(tensors: Sequence[torch.Tensor], scales: Sequence[float]):
+    """Descriptors for logical-[N,C,H,W] tensors of any strides (NCHW or channels-last views)."""
+    arr = (RafLevel * len(tensors))()
+    for i, (t, s) in enumerate(zip(tensors, scales)):
+        assert t.dim() == 4
+        arr[i].data = t.data_ptr()
+        arr[i].n, arr[i].c, arr[i].h, arr[i].w = t.shape
+        arr[i].sn, arr[i].sc, arr[i].sh, arr[i].sw = t.stride()
+        arr[i].spatial_scale = float(s)
+    return arr
+
+
+def _strides4(t: torch.Tensor):
+    assert t.dim() == 4
+    return (ctypes.c_int64 * 4)(*t.stride())
+
+
+def roi_align_fpn_workspace_bytes(K: int, L: int, out_h: int, out_w: int, sampling_ratio: int,
+                                  flags: int = 0) -> int:
+    return int(lib().roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
+
+
+def roi_fpn_assign_levels(rois: torch.Tensor, L: int, finest_scale: float,
+                          levels: Optional[torch.Tensor], counts: Optional[torch.Tensor],
+                          perm: Optional[torch.Tensor], ws: Optional[torch.Tensor] = None,
+                          stream=None) -> None:
+    K = rois.shape[0]
+    rc = lib().roi_fpn_assign_levels(_ptr(rois), K, L, finest_scale, _ptr(levels), _ptr(counts),
+                                     _ptr(perm), _ptr(ws), 0 if ws is None else ws.numel() * ws.element_size(),
+                                     _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_fpn_assign_levels")
+
+
+def roi_align_fpn_forward(feats: Sequence[torch.Tensor], scales: Sequence[float], rois: torch.Tensor,
+                          out: torch.Tensor, sampling_ratio: int, aligned: bool, finest_scale: float,
+                          ws: torch.Tensor, stream=None, levels_desc=None) -> None:
+    """out: logical [K,C,PH,PW] tensor of any strides (e.g. a permuted view of a [K,PH,PW,C] buffer)."""
+    desc = levels_desc if levels_desc is not None else make_levels(feats, scales)
+    K, _, PH, PW = out.shape
+    rc = lib().roi_align_fpn_forward(desc, len(feats), _DTYPES[feats[0].dtype], _ptr(rois), K, PH, PW,
+                                     sampling_ratio, int(bool(aligned)), finest_scale, _ptr(out),
+                                     _strides4(out), _ptr(ws), ws.numel() * ws.element_size(),
+                                     _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fpn_forward")
+
+
+def roi_align_fpn_backward(grad_feats: Sequence[torch.Tensor], scales: Sequence[float],
+                           grad_out: torch.Tensor, rois: torch.Tensor, sampling_ratio: int,
+                           aligned: bool, finest_scale: float, flags: int, ws: torch.Tensor,
+                           stream=None, levels_desc=None) -> None:
+    desc = levels_desc if levels_desc is not None else make_levels(grad_feats, scales)
+    K, _, PH, PW = grad_out.shape
+    rc = lib().roi_align_fpn_backward(desc, len(grad_feats), _DTYPES[grad_out.dtype], _ptr(grad_out),
+                                      _strides4(grad_out), _ptr(rois), K, PH, PW, sampling_ratio,
+                                      int(bool(aligned)), finest_scale, flags, _ptr(ws),
+                                      ws.numel() * ws.element_size(), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fpn_backward")
+
+
+def roi_align_fpn_host_arena_bytes(levels: Sequence[torch.Tensor], scales, dtype: torch.dtype, K: int,
+                                   out_h: int, out_w: int, sampling_ratio: int, flags: int = 0) -> int:
+    desc = make_levels(levels, scales)
+    return int(lib().roi_align_fpn_host_arena_bytes(desc, len(levels), _DTYPES[dtype], K, out_h, out_w,
+                                                    sampling_ratio, flags))
+
+
+def roi_align_fpn_forward_host(feats_host: Sequence[torch.Tensor], scales, rois_host: torch.Tensor,
+                               out_host: torch.Tensor, sampling_ratio: int, aligned: bool,
+                               finest_scale: float, arena: torch.Tensor, stream=None) -> None:
+    """HOST (pinned) tensors in and out; `arena` is a device byte buffer."""
+    desc = make_levels(feats_host, scales)
+    K, _, PH, PW = out_host.shape
+    rc = lib().roi_align_fpn_forward_host(desc, len(feats_host), _DTYPES[feats_host[0].dtype],
+                                          _ptr(rois_host), K, PH, PW, sampling_ratio, int(bool(aligned)),
+                                          finest_scale, _ptr(out_host), _strides4(out_host), _ptr(arena),
+                                          arena.numel() * arena.element_size(), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fpn_forward_host")
+
+
+def roi_align_fpn_backward_host(grad_feats_host: Sequence[torch.Tensor], scales,
+                                grad_out_host: torch.Tensor, rois_host: torch.Tensor,
+                                sampling_ratio: int, aligned: bool, finest_scale: float, flags: int,
+                                arena: torch.Tensor, stream=None) -> None:
+    desc = make_levels(grad_feats_host, scales)
+    K, _, PH, PW = grad_out_host.shape
+    rc = lib().roi_align_fpn_backward_host(desc, len(grad_feats_host), _DTYPES[grad_out_host.dtype],
+                                           _ptr(grad_out_host), _strides4(grad_out_host), _ptr(rois_host),
+                                           K, PH, PW, sampling_ratio, int(bool(aligned)), finest_scale,
+                                           flags, _ptr(arena), arena.numel() * arena.element_size(),
+                                           _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fpn_backward_host")

@@ -1,0 +1,291 @@
+// raf_api.cu -- the C ABI of libraf.so (include/raf.h): argument validation, layout
+// classification and kernel dispatch.  No allocation, no synchronisation, no device->host copy
+// (except the documented *_host entry points, which copy between caller-owned buffers).
+#include <atomic>
+#include <cstring>
+
+#include "raf_device.cuh"
+#include "raf_host.h"
+
+namespace raf {
+
+static std::atomic<uint64_t> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+static size_t esize(raf_dtype d) { return d == RAF_F32 ? 4 : 2; }
+
+static int check_levels(const raf_level* lv, int L) {
+  if (!lv) return RAF_ERR_NULL;
+  if (L < 1 || L > kMaxLevels) return RAF_ERR_SHAPE;
+  for (int l = 0; l < L; ++l) {
+    if (!lv[l].data) return RAF_ERR_NULL;
+    if (lv[l].n < 1 || lv[l].c < 1 || lv[l].h < 1 || lv[l].w < 1) return RAF_ERR_SHAPE;
+    if (lv[l].n != lv[0].n || lv[l].c != lv[0].c) return RAF_ERR_SHAPE;
+    if (lv[l].sn <= 0 || lv[l].sc <= 0 || lv[l].sh <= 0 || lv[l].sw <= 0) return RAF_ERR_STRIDE;
+    if (!(lv[l].spatial_scale > 0.0f)) return RAF_ERR_SHAPE;
+  }
+  return RAF_OK;
+}
+
+static int check_common(const float* rois, int K, int out_h, int out_w, int sampling_ratio) {
+  if (K < 0 || out_h < 1 || out_h > 32 || out_w < 1 || out_w > 32) return RAF_ERR_SHAPE;
+  if (sampling_ratio < 0 || sampling_ratio > 16) return RAF_ERR_SHAPE;
+  if (K > 0 && !rois) return RAF_ERR_NULL;
+  return RAF_OK;
+}
+
+static void fill_param(const raf_level* lv, int L, LevelsParam* p) {
+  std::memset(p, 0, sizeof(*p));
+  p->n = lv[0].n; p->c = lv[0].c; p->L = L;
+  for (int l = 0; l < L; ++l) {
+    p->data[l] = lv[l].data;
+    p->sn[l] = lv[l].sn; p->sc[l] = lv[l].sc; p->sh[l] = lv[l].sh; p->sw[l] = lv[l].sw;
+    p->h[l] = lv[l].h; p->w[l] = lv[l].w; p->scale[l] = lv[l].spatial_scale;
+  }
+}
+
+// Channels-last fast-path eligibility: unit channel stride, `vec`-element (16-byte for the
+// features, see callers) aligned pixel vectors, in-image offsets that fit int32.
+static bool levels_vectorizable(const raf_level* lv, int L, int vec, size_t elem) {
+  for (int l = 0; l < L; ++l) {
+    if (lv[l].sc != 1 || lv[l].c % vec) return false;
+    if (lv[l].sn % vec || lv[l].sh % vec || lv[l].sw % vec) return false;
+    if (((uintptr_t)lv[l].data) % (vec * elem)) return false;
+    const int64_t span = (int64_t)(lv[l].h - 1) * lv[l].sh + (int64_t)(lv[l].w - 1) * lv[l].sw + lv[l].c;
+    if (span >= ((int64_t)1 << 31)) return false;
+  }
+  return true;
+}
+
+static bool tensor_vectorizable(const void* p, const int64_t* s, int vec, size_t elem) {
+  return s[1] == 1 && s[0] % vec == 0 && s[2] % vec == 0 && s[3] % vec == 0 &&
+         ((uintptr_t)p) % (vec * elem) == 0;
+}
+
+// A level is one dense block when its strides are a permutation of a packed layout.
+static bool level_dense(const raf_level& v) {
+  int64_t ext[4] = {v.n, v.c, v.h, v.w}, st[4] = {v.sn, v.sc, v.sh, v.sw};
+  for (int i = 0; i < 4; ++i)
+    for (int j = i + 1; j < 4; ++j)
+      if (st[j] < st[i] || (st[j] == st[i] && ext[j] < ext[i])) {
+        std::swap(st[i], st[j]); std::swap(ext[i], ext[j]);
+      }
+  int64_t run = 1;
+  for (int i = 0; i < 4; ++i) {
+    if (ext[i] == 1) continue;
+    if (st[i] != run) return false;
+    run *= ext[i];
+  }
+  return true;
+}
+
+}  // namespace raf
+
+using namespace raf;
+
+extern "C" {
+
+size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,
+                                     int flags) {
+  (void)L; (void)out_h; (void)out_w; (void)sampling_ratio; (void)flags;
+  const size_t k = K > 0 ? (size_t)K : 0;
+  // [levels K][perm K][counts 8] int32, each 256-aligned
+  return 256 + 2 * align256(4 * k) + 256;
+}
+
+int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
+                          int32_t* counts, int32_t* perm, void* ws, size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  if (K < 0 || L < 1 || L > kMaxLevels) return RAF_ERR_SHAPE;
+  if (K > 0 && !rois) return RAF_ERR_NULL;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
+  if (K == 0 && !counts) return RAF_OK;
+  return launch_assign_levels(rois, K, L, finest_scale, levels, counts, perm, (cudaStream_t)stream);
+}
+
+int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                          int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
+                          void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,
+                          void* stream) {
+  int rc = check_levels(feats, L);
+  if (rc) return rc;
+  rc = check_common(rois, K, out_h, out_w, sampling_ratio);
+  if (rc) return rc;
+  if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
+  if (!out_strides) return RAF_ERR_NULL;
+  for (int i = 0; i < 4; ++i) if (out_strides[i] <= 0) return RAF_ERR_STRIDE;
+  if (K == 0) return RAF_OK;
+  if (!out) return RAF_ERR_NULL;
+  if (!ws) return RAF_ERR_NULL;
+  if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, 0)) return RAF_ERR_WORKSPACE;
+
+  LevelsParam p;
+  fill_param(feats, L, &p);
+  const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
+  const int vec = (int)(16 / esize(dtype));
+  const bool cl = levels_vectorizable(feats, L, vec, esize(dtype)) &&
+                  tensor_vectorizable(out, out_strides, vec, esize(dtype));
+  return launch_forward(p, dtype, a, out, out_strides, cl, (cudaStream_t)stream);
+}
+
+int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
+                           const void* grad_out, const int64_t* gout_strides, const float* rois,
+                           int K, int out_h, int out_w, int sampling_ratio, int aligned,
+                           float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream) {
+  int rc = check_levels(grad_feats, L);
+  if (rc) return rc;
+  rc = check_common(rois, K, out_h, out_w, sampling_ratio);
+  if (rc) return rc;
+  if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC)) return RAF_ERR_UNSUPPORTED;
+  if (!gout_strides) return RAF_ERR_NULL;
+  for (int i = 0; i < 4; ++i) if (gout_strides[i] <= 0) return RAF_ERR_STRIDE;
+  if (K > 0 && !grad_out) return RAF_ERR_NULL;
+  if (K > 0 && !ws) return RAF_ERR_NULL;
+  if (K > 0 && ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
+    return RAF_ERR_WORKSPACE;
+  if (flags & RAF_DETERMINISTIC) return RAF_ERR_UNSUPPORTED;  // K3d: not in this build yet
+  cudaStream_t st = (cudaStream_t)stream;
+
+  if (!(flags & RAF_ACCUMULATE)) {
+    for (int l = 0; l < L; ++l) {
+      const raf_level& v = grad_feats[l];
+      if (level_dense(v)) {
+        if (cudaMemsetAsync(v.data, 0, sizeof(float) * (size_t)v.n * v.c * v.h * v.w, st) != cudaSuccess)
+          return RAF_ERR_CUDA;
+        count_launch();
+      } else {
+        rc = launch_zero_level((float*)v.data, v.n, v.c, v.h, v.w, v.sn, v.sc, v.sh, v.sw, st);
+        if (rc) return rc;
+      }
+    }
+  }
+  if (K == 0) return RAF_OK;
+
+  LevelsParam p;
+  fill_param(grad_feats, L, &p);
+  const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
+  const bool cl = levels_vectorizable(grad_feats, L, 4, 4) &&
+                  tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype));
+  return launch_backward_atomic(p, gout_dtype, a, grad_out, gout_strides, cl, st);
+}
+
+// ---- end-to-end variants with HOST buffers -----------------------------------------------------
+static bool tensor_dense(int K, int C, int PH, int PW, const int64_t* s) {
+  raf_level v;
+  v.n = K; v.c = C; v.h = PH; v.w = PW; v.sn = s[0]; v.sc = s[1]; v.sh = s[2]; v.sw = s[3];
+  return level_dense(v);
+}
+
+size_t roi_align_fpn_host_arena_bytes(const raf_level* levels, int L, raf_dtype dtype, int K,
+                                      int out_h, int out_w, int sampling_ratio, int flags) {
+  if (!levels || L < 1 || L > kMaxLevels || K < 0) return 0;
+  size_t total = 256;
+  for (int l = 0; l < L; ++l)   // features (dtype) or gradients (fp32): size for the larger
+    total += align256((size_t)levels[l].n * levels[l].c * levels[l].h * levels[l].w * 4);
+  total += align256((size_t)K * 20);
+  total += align256((size_t)K * levels[0].c * out_h * out_w * esize(dtype));
+  total += roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags);
+  return total;
+}
+
+int roi_align_fpn_forward_host(const raf_level* feats_host, int L, raf_dtype dtype,
+                               const float* rois_host, int K, int out_h, int out_w,
+                               int sampling_ratio, int aligned, float finest_scale, void* out_host,
+                               const int64_t* out_strides, void* arena, size_t arena_bytes,
+                               void* stream) {
+  int rc = check_levels(feats_host, L);
+  if (rc) return rc;
+  if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (K < 0 || out_h < 1 || out_w < 1) return RAF_ERR_SHAPE;
+  if (!out_strides || !arena || (K > 0 && (!rois_host || !out_host))) return RAF_ERR_NULL;
+  if (arena_bytes < roi_align_fpn_host_arena_bytes(feats_host, L, dtype, K, out_h, out_w, sampling_ratio, 0))
+    return RAF_ERR_WORKSPACE;
+  if (!tensor_dense(K, feats_host[0].c, out_h, out_w, out_strides)) return RAF_ERR_STRIDE;
+  cudaStream_t st = (cudaStream_t)stream;
+  char* cur = (char*)arena;
+  raf_level dev[kMaxLevels];
+  for (int l = 0; l < L; ++l) {
+    if (!level_dense(feats_host[l])) return RAF_ERR_STRIDE;
+    const size_t bytes = (size_t)feats_host[l].n * feats_host[l].c * feats_host[l].h * feats_host[l].w * esize(dtype);
+    dev[l] = feats_host[l];
+    dev[l].data = cur;
+    if (cudaMemcpyAsync(cur, feats_host[l].data, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return RAF_ERR_CUDA;
+    cur += align256(bytes);
+  }
+  float* d_rois = (float*)cur;
+  if (K > 0 && cudaMemcpyAsync(d_rois, rois_host, (size_t)K * 20, cudaMemcpyHostToDevice, st) != cudaSuccess) return RAF_ERR_CUDA;
+  cur += align256((size_t)K * 20);
+  void* d_out = cur;
+  const size_t out_bytes = (size_t)K * feats_host[0].c * out_h * out_w * esize(dtype);
+  cur += align256(out_bytes);
+  const size_t ws_bytes = roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, 0);
+  rc = roi_align_fpn_forward(dev, L, dtype, d_rois, K, out_h, out_w, sampling_ratio, aligned,
+                             finest_scale, d_out, out_strides, cur, ws_bytes, stream);
+  if (rc) return rc;
+  if (K > 0 && cudaMemcpyAsync(out_host, d_out, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return RAF_ERR_CUDA;
+  return RAF_OK;
+}
+
+int roi_align_fpn_backward_host(const raf_level* grad_feats_host, int L, raf_dtype gout_dtype,
+                                const void* grad_out_host, const int64_t* gout_strides,
+                                const float* rois_host, int K, int out_h, int out_w,
+                                int sampling_ratio, int aligned, float finest_scale, int flags,
+                                void* arena, size_t arena_bytes, void* stream) {
+  int rc = check_levels(grad_feats_host, L);
+  if (rc) return rc;
+  if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (K < 0 || out_h < 1 || out_w < 1) return RAF_ERR_SHAPE;
+  if (!gout_strides || !arena || (K > 0 && (!rois_host || !grad_out_host))) return RAF_ERR_NULL;
+  if (arena_bytes < roi_align_fpn_host_arena_bytes(grad_feats_host, L, gout_dtype, K, out_h, out_w, sampling_ratio, flags))
+    return RAF_ERR_WORKSPACE;
+  if (!tensor_dense(K, grad_feats_host[0].c, out_h, out_w, gout_strides)) return RAF_ERR_STRIDE;
+  cudaStream_t st = (cudaStream_t)stream;
+  char* cur = (char*)arena;
+  raf_level dev[kMaxLevels];
+  size_t lbytes[kMaxLevels];
+  for (int l = 0; l < L; ++l) {
+    if (!level_dense(grad_feats_host[l])) return RAF_ERR_STRIDE;
+    lbytes[l] = (size_t)grad_feats_host[l].n * grad_feats_host[l].c * grad_feats_host[l].h * grad_feats_host[l].w * 4;
+    dev[l] = grad_feats_host[l];
+    dev[l].data = cur;
+    if ((flags & RAF_ACCUMULATE) &&
+        cudaMemcpyAsync(cur, grad_feats_host[l].data, lbytes[l], cudaMemcpyHostToDevice, st) != cudaSuccess) return RAF_ERR_CUDA;
+    cur += align256(lbytes[l]);
+  }
+  float* d_rois = (float*)cur;
+  if (K > 0 && cudaMemcpyAsync(d_rois, rois_host, (size_t)K * 20, cudaMemcpyHostToDevice, st) != cudaSuccess) return RAF_ERR_CUDA;
+  cur += align256((size_t)K * 20);
+  void* d_gout = cur;
+  const size_t gout_bytes = (size_t)K * grad_feats_host[0].c * out_h * out_w * esize(gout_dtype);
+  if (K > 0 && cudaMemcpyAsync(d_gout, grad_out_host, gout_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return RAF_ERR_CUDA;
+  cur += align256(gout_bytes);
+  const size_t ws_bytes = roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags);
+  rc = roi_align_fpn_backward(dev, L, gout_dtype, d_gout, gout_strides, d_rois, K, out_h, out_w,
+                              sampling_ratio, aligned, finest_scale, flags, cur, ws_bytes, stream);
+  if (rc) return rc;
+  for (int l = 0; l < L; ++l)
+    if (cudaMemcpyAsync(grad_feats_host[l].data, dev[l].data, lbytes[l], cudaMemcpyDeviceToHost, st) != cudaSuccess) return RAF_ERR_CUDA;
+  return RAF_OK;
+}
+
+const char* roi_align_fpn_strerror(int status) {
+  switch (status) {
+    case RAF_OK: return "ok";
+    case RAF_ERR_NULL: return "a required pointer is NULL";
+    case RAF_ERR_SHAPE: return "invalid shape / size / count argument";
+    case RAF_ERR_DTYPE: return "unknown dtype";
+    case RAF_ERR_STRIDE: return "invalid stride";
+    case RAF_ERR_UNSUPPORTED: return "valid request not supported by this build";
+    case RAF_ERR_WORKSPACE: return "workspace too small";
+    case RAF_ERR_CUDA: return "CUDA runtime error";
+  }
+  return "unknown status";
+}
+
+uint64_t roi_align_fpn_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

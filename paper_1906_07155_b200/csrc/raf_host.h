@@ -1,0 +1,41 @@
+// raf_host.h -- internal host-side declarations shared by the raf translation units.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/raf.h"
+
+namespace raf {
+
+struct LevelsParam;
+
+// Common per-call arguments of the RoIAlign kernels.
+struct RoiArgs {
+  const float* rois;
+  int K;
+  int PH, PW;
+  int sampling_ratio;
+  int aligned;
+  float finest_scale;
+};
+
+void count_launch();
+
+int launch_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
+                         int32_t* counts, int32_t* perm, cudaStream_t stream);
+
+// Forward.  `channels_last` = every level has sc == 1 and the output has stride 1 along C, with
+// 16-byte aligned pixel vectors (checked by the caller).
+int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
+                   const int64_t* out_strides, bool channels_last, cudaStream_t stream);
+
+// Backward (atomic scatter).  The gradient pyramid must already hold its starting values.
+int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a,
+                           const void* grad_out, const int64_t* gout_strides, bool channels_last,
+                           cudaStream_t stream);
+
+// Zero-fill of one strided level (used when the level is not one dense block).
+int launch_zero_level(float* data, int n, int c, int h, int w, int64_t sn, int64_t sc, int64_t sh,
+                      int64_t sw, cudaStream_t stream);
+
+}  // namespace raf

@@ -1,0 +1,262 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Level assignment / bucketing bit-exact; forward and backward within the
+tolerances of readings S10 / S11 (BASELINE.json north_star)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import raf_ref as R
+from paper_1906_07155_b200 import binding as B
+from paper_1906_07155_b200 import inputs
+import raf_testlib as T
+
+pytestmark = pytest.mark.gpu
+
+
+# ------------------------------------------------------------------------------------------------
+# K1: levels / histogram / stable bucketing -- bit exact
+# ------------------------------------------------------------------------------------------------
+def _gpu_levels(rois_np, L, fs):
+    K = rois_np.shape[0]
+    rois = torch.from_numpy(np.ascontiguousarray(rois_np, np.float32)).cuda()
+    levels = torch.full((max(K, 1),), -7, dtype=torch.int32, device="cuda")
+    counts = torch.full((L,), -7, dtype=torch.int32, device="cuda")
+    perm = torch.full((max(K, 1),), -7, dtype=torch.int32, device="cuda")
+    B.roi_fpn_assign_levels(rois, L, fs, levels, counts, perm)
+    torch.cuda.synchronize()
+    return levels[:K].cpu().numpy(), counts.cpu().numpy(), perm[:K].cpu().numpy()
+
+
+@pytest.mark.parametrize("index", [2, 3, 4, 5])
+def test_levels_bit_exact_configs(index):
+    wl = inputs.make_workload(index, with_feats=False, with_grad=False)
+    got = _gpu_levels(wl.rois, 4, 56.0)
+    ref = R.assign_levels(wl.rois, 4, 56.0)
+    for g, r in zip(got, ref):
+        assert np.array_equal(g, r)
+    assert got[1].tolist() == list(wl.cfg.level_hist)
+
+
+@pytest.mark.parametrize("L,fs", [(4, 56.0), (1, 56.0), (2, 56.0), (8, 7.0), (5, 33.3)])
+def test_levels_bit_exact_adversarial(L, fs):
+    rois = inputs.adversarial_level_rois(fs, min(L, 6))
+    rng = np.random.default_rng(1)
+    rois = rois[rng.permutation(len(rois))]          # shuffled: stability must not rely on order
+    got = _gpu_levels(rois, L, fs)
+    ref = R.assign_levels(rois, L, fs)
+    for g, r in zip(got, ref):
+        assert np.array_equal(g, r)
+
+
+@pytest.mark.parametrize("K", [0, 1, 31, 1024, 1025, 5000])
+def test_levels_sizes_and_ragged_tail(K):
+    rng = np.random.default_rng(K)
+    side = np.exp(rng.uniform(np.log(8), np.log(1500), K))
+    rois = np.stack([np.zeros(K), np.zeros(K), np.zeros(K), side, side * rng.uniform(0.5, 2, K)], 1).astype(np.float32)
+    got = _gpu_levels(rois, 4, 56.0)
+    ref = R.assign_levels(rois, 4, 56.0)
+    for g, r in zip(got, ref):
+        assert np.array_equal(g, r)
+
+
+# ------------------------------------------------------------------------------------------------
+# K2 forward
+# ------------------------------------------------------------------------------------------------
+def _fwd_case(wl, dtype, layout, P=None, g=None, aligned=None):
+    cfg = wl.cfg
+    P = P or cfg.out_size
+    g = cfg.sampling_ratio if g is None else g
+    aligned = cfg.aligned if aligned is None else aligned
+    dev, exact = T.device_feats(wl.feats, dtype, layout)
+    got = T.gpu_forward(dev, cfg.scales, wl.rois, P, g, aligned, cfg.finest_scale, layout)
+    ref = R.forward(exact, cfg.scales, wl.rois, P, g, aligned, cfg.finest_scale, coord_f32=True)
+    return T.assert_forward_close(got, ref, dtype)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+def test_forward_config1(layout):
+    _fwd_case(inputs.make_workload(1), "f32", layout)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("index,dtype,kw", [
+    (2, "f32", dict(n_img=2, per_img=96)),
+    (3, "f16", dict(n_img=1, per_img=150)),
+    (4, "bf16", dict(n_img=2, per_img=40)),
+    (5, "bf16", dict(n_img=3, per_img=64)),     # boxes partly outside the image
+    (5, "f32", dict(n_img=2, per_img=50, channels=36)),   # C not a multiple of 32 lanes
+])
+def test_forward_reduced_configs(index, dtype, kw, layout):
+    _fwd_case(inputs.make_workload(index, **kw), dtype, layout)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("P,g,aligned", [((7, 7), 1, True), ((7, 7), 3, True), ((7, 7), 0, True),
+                                         ((7, 7), 2, False), ((7, 7), 0, False), ((5, 9), 2, True),
+                                         ((1, 1), 4, True), ((14, 14), 2, False), ((32, 32), 2, True),
+                                         ((3, 2), 16, True)])
+def test_forward_variants(P, g, aligned, layout):
+    wl = inputs.make_workload(5, n_img=2, per_img=24, channels=8)
+    _fwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned)
+
+
+def test_forward_degenerate_and_invalid_rois():
+    wl = inputs.make_workload(2, n_img=2, per_img=8, channels=16)
+    rois = np.array([[0, 100, 100, 100, 100], [1, 300, 200, 100, 50], [0, -500, -500, -400, -400],
+                     [1, 0, 0, 1344, 800], [2, 10, 10, 90, 90], [-1, 10, 10, 90, 90],
+                     [0.5, 10, 10, 90, 90], [0, 1343.9, 799.9, 1344, 800], [1, 5000, 5000, 6000, 6000]], np.float32)
+    wl.rois = rois
+    for layout in ("cl", "nchw"):
+        dev, exact = T.device_feats(wl.feats, "f32", layout)
+        got = T.gpu_forward(dev, wl.cfg.scales, rois, (7, 7), 2, True, 56.0, layout)
+        ref = R.forward(exact, wl.cfg.scales, rois, (7, 7), 2, True, 56.0, coord_f32=True)
+        T.assert_forward_close(got, ref, "f32")
+        assert np.all(got[4:7] == 0)     # invalid batch index -> zero rows (reading S17)
+
+
+def test_forward_metamorphic_layouts_and_permutation():
+    wl = inputs.make_workload(2, n_img=2, per_img=64, channels=64)
+    cfg = wl.cfg
+    outs = {}
+    for layout in ("cl", "nchw"):
+        dev, _ = T.device_feats(wl.feats, "f32", layout)
+        outs[layout] = T.gpu_forward(dev, cfg.scales, wl.rois, (7, 7), 2, True, 56.0, layout)
+    # same coordinates and weights in both kernels; only the accumulation order may differ
+    assert np.abs(outs["cl"] - outs["nchw"]).max() < 2e-6
+    p = np.random.default_rng(0).permutation(cfg.K)
+    dev, _ = T.device_feats(wl.feats, "f32", "cl")
+    shuffled = T.gpu_forward(dev, cfg.scales, wl.rois[p], (7, 7), 2, True, 56.0, "cl")
+    assert np.array_equal(shuffled, outs["cl"][p])
+    # channel slicing: a strided channel slice of the channels-last buffer (generic path) agrees
+    dev_slice = [d[:, 8:24] for d in dev]
+    sl = T.gpu_forward(dev_slice, cfg.scales, wl.rois, (7, 7), 2, True, 56.0, "cl")
+    assert np.abs(sl - outs["cl"][:, 8:24]).max() < 2e-6
+
+
+@pytest.mark.parametrize("index", [2, 3, 4, 5])
+def test_forward_full_size_sampled(index):
+    """BASELINE.json full sizes in the layout bench.py times; the oracle recomputes a sample of RoIs
+    (rows are independent, so row k of the full run must equal the oracle on rois[k])."""
+    wl = inputs.make_workload(index, with_grad=False)
+    cfg = wl.cfg
+    dev, _ = T.device_feats(wl.feats, cfg.dtype, "cl")
+    got = T.gpu_forward(dev, cfg.scales, wl.rois, cfg.out_size, 2, True, 56.0, "cl")
+    assert np.isfinite(got).all()
+    rng = np.random.default_rng(index)
+    pick = np.sort(rng.choice(cfg.K, 48, replace=False))
+    exact = [d.permute(0, 1, 2, 3).to(torch.float64).cpu().numpy() for d in dev]
+    ref = R.forward(exact, cfg.scales, wl.rois[pick], cfg.out_size, 2, True, 56.0, coord_f32=True)
+    T.assert_forward_close(got[pick], ref, cfg.dtype)
+
+
+# ------------------------------------------------------------------------------------------------
+# K3 backward
+# ------------------------------------------------------------------------------------------------
+def _bwd_case(wl, gout_dtype, layout, P=None, g=None, aligned=None, flags=0, init=None):
+    cfg = wl.cfg
+    P = P or cfg.out_size
+    g = cfg.sampling_ratio if g is None else g
+    aligned = cfg.aligned if aligned is None else aligned
+    gout = wl.grad_out
+    if gout.shape[2:] != tuple(P):
+        gout = np.random.default_rng(5).standard_normal((cfg.K, cfg.channels, *P)).astype(np.float32)
+    got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, gout, wl.rois, g, aligned, cfg.finest_scale,
+                                   layout, gout_dtype, flags, init)
+    ref, S = R.backward(cfg.level_shapes, cfg.scales, go_exact, wl.rois, P, g, aligned, cfg.finest_scale,
+                        coord_f32=True, accumulate_into=init)
+    if init is not None:   # starting values count towards the error scale
+        S = [s + np.abs(i) for s, i in zip(S, init)]
+    return T.assert_backward_close(got, ref, S)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+def test_backward_config1(layout):
+    _bwd_case(inputs.make_workload(1), "f32", layout)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("index,dtype,kw", [
+    (2, "f32", dict(n_img=2, per_img=96, channels=64)),
+    (4, "bf16", dict(n_img=2, per_img=40, channels=32)),
+    (5, "bf16", dict(n_img=3, per_img=64, channels=32)),
+    (5, "f16", dict(n_img=2, per_img=50, channels=36)),
+])
+def test_backward_reduced_configs(index, dtype, kw, layout):
+    _bwd_case(inputs.make_workload(index, **kw), dtype, layout)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("P,g,aligned", [((7, 7), 1, True), ((7, 7), 0, True), ((7, 7), 2, False),
+                                         ((5, 9), 3, True), ((14, 14), 2, True), ((7, 7), 0, False)])
+def test_backward_variants(P, g, aligned, layout):
+    wl = inputs.make_workload(5, n_img=2, per_img=24, channels=8)
+    _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned)
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+def test_backward_accumulate_mode(layout):
+    wl = inputs.make_workload(2, n_img=2, per_img=32, channels=16)
+    rng = np.random.default_rng(3)
+    init = [rng.standard_normal(s).astype(np.float32).astype(np.float64) for s in wl.cfg.level_shapes]
+    _bwd_case(wl, "f32", layout, flags=B.RAF_ACCUMULATE, init=init)
+
+
+def test_backward_full_size_config2():
+    wl = inputs.make_workload(2, with_feats=False)
+    cfg = wl.cfg
+    got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl")
+    # the oracle on a channel slice (channels are independent)
+    sl = slice(40, 56)
+    shapes = [(s[0], 16, s[2], s[3]) for s in cfg.level_shapes]
+    ref, S = R.backward(shapes, cfg.scales, go_exact[:, sl], wl.rois, (7, 7), 2, True, 56.0)
+    T.assert_backward_close([g[:, sl] for g in got], ref, S)
+    # properties that hold at any size: total mass and untouched pixels
+    masks = R.footprint(cfg.level_shapes, cfg.scales, wl.rois, (7, 7), 2, True)
+    for g, m in zip(got, masks):
+        assert np.all(g[np.broadcast_to(m[:, None] == 0, g.shape)] == 0)
+
+
+def test_adjoint_identity_on_gpu():
+    """<A x, g> = <x, A^T g> with both sides from the CUDA path (fp32): a property at full config-2
+    size that needs no oracle."""
+    wl = inputs.make_workload(2)
+    cfg = wl.cfg
+    dev, _ = T.device_feats(wl.feats, "f32", "cl")
+    out = T.gpu_forward(dev, cfg.scales, wl.rois, (7, 7), 2, True, 56.0, "cl")
+    grads, go = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl")
+    lhs = float((out * go).sum())
+    rhs = sum(float((g * f.astype(np.float64)).sum()) for g, f in zip(grads, wl.feats))
+    scale = float(np.abs(out * go).sum())
+    assert abs(lhs - rhs) <= 1e-5 * scale
+
+
+# ------------------------------------------------------------------------------------------------
+# ABI behaviour on the device
+# ------------------------------------------------------------------------------------------------
+def test_k_zero_and_overwrite_zero_fill():
+    shapes = [(1, 8, 10, 12), (1, 8, 5, 6)]
+    grads, _ = T.gpu_backward(shapes, [0.25, 0.125], np.zeros((0, 8, 7, 7), np.float32),
+                              np.zeros((0, 5), np.float32), 2, True, 56.0, "cl")
+    assert all(np.all(g == 0) for g in grads)      # overwrite mode writes every element
+
+
+def test_host_entry_points_match_device_path():
+    wl = inputs.make_workload(2, n_img=1, per_img=32, channels=32)
+    cfg = wl.cfg
+    feats_h = [torch.from_numpy(f).permute(0, 2, 3, 1).contiguous().pin_memory().permute(0, 3, 1, 2) for f in wl.feats]
+    rois_h = torch.from_numpy(wl.rois).pin_memory()
+    out_h = torch.empty((cfg.K, 7, 7, 32), dtype=torch.float32).pin_memory().permute(0, 3, 1, 2)
+    nbytes = B.roi_align_fpn_host_arena_bytes(feats_h, cfg.scales, torch.float32, cfg.K, 7, 7, 2)
+    arena = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    B.roi_align_fpn_forward_host(feats_h, cfg.scales, rois_h, out_h, 2, True, 56.0, arena)
+    torch.cuda.synchronize()
+    dev, _ = T.device_feats(wl.feats, "f32", "cl")
+    ref = T.gpu_forward(dev, cfg.scales, wl.rois, (7, 7), 2, True, 56.0, "cl")
+    assert np.array_equal(out_h.numpy().astype(np.float64), ref)
+    gout_h = torch.from_numpy(wl.grad_out).permute(0, 2, 3, 1).contiguous().pin_memory().permute(0, 3, 1, 2)
+    grads_h = [torch.empty((s[0], s[2], s[3], s[1]), dtype=torch.float32).pin_memory().permute(0, 3, 1, 2)
+               for s in cfg.level_shapes]
+    B.roi_align_fpn_backward_host(grads_h, cfg.scales, gout_h, rois_h, 2, True, 56.0, 0, arena)
+    torch.cuda.synchronize()
+    ref_g, S = R.backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, (7, 7), 2, True, 56.0)
+    T.assert_backward_close([g.numpy().astype(np.float64) for g in grads_h], ref_g, S)

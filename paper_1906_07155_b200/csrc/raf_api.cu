@@ -115,8 +115,8 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
   if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
   if (!out_strides) return RAF_ERR_NULL;
+  if (K == 0) return RAF_OK;  // nothing to do; strides of an empty tensor are not meaningful
   for (int i = 0; i < 4; ++i) if (out_strides[i] <= 0) return RAF_ERR_STRIDE;
-  if (K == 0) return RAF_OK;
   if (!out) return RAF_ERR_NULL;
   if (!ws) return RAF_ERR_NULL;
   if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, 0)) return RAF_ERR_WORKSPACE;
@@ -142,7 +142,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
   if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC)) return RAF_ERR_UNSUPPORTED;
   if (!gout_strides) return RAF_ERR_NULL;
-  for (int i = 0; i < 4; ++i) if (gout_strides[i] <= 0) return RAF_ERR_STRIDE;
+  for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
   if (K > 0 && !grad_out) return RAF_ERR_NULL;
   if (K > 0 && !ws) return RAF_ERR_NULL;
   if (K > 0 && ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))

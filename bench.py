@@ -37,7 +37,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based)")
     ap.add_argument("--layout", default="cl", choices=["cl", "nchw"])
-    ap.add_argument("--deterministic", action="store_true", help="time the RAF_DETERMINISTIC backward")
+    ap.add_argument("--backward", default="auto", choices=["auto", "atomic", "deterministic"],
+                    help="auto: library's choice (pull when eligible); atomic: RAF_ATOMIC; deterministic: RAF_DETERMINISTIC")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--graph", action="store_true", help="replay each step from a CUDA graph")
@@ -208,7 +209,7 @@ def run_ours(args):
     K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
     PH, PW = cfg.out_size
     g, aligned, fs = cfg.sampling_ratio, cfg.aligned, cfg.finest_scale
-    flags = B.RAF_DETERMINISTIC if args.deterministic else 0
+    flags = {"auto": 0, "atomic": B.RAF_ATOMIC, "deterministic": B.RAF_DETERMINISTIC}[args.backward]
 
     def lay(t):   # logical NCHW tensor -> requested physical layout
         return t.contiguous() if args.layout == "nchw" else t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
@@ -288,7 +289,7 @@ def run_ours(args):
         dist.barrier()
     launches = B.launch_count() - launches0
     if graphs:   # replayed launches are not seen by the library's counter: count per captured step
-        launches = args.steps * (1 + (1 + L) * cfg.backward)
+        launches = args.steps * (1 + ((1 + L) if args.backward == "atomic" else 2) * cfg.backward)
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     if world > 1:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
@@ -330,7 +331,7 @@ def run_ours(args):
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {cfg.name}", "K": K, "C": C,
                        "out_size": [PH, PW], "levels": L, "layout": args.layout, "parallelism": f"replicas x{world} (shard by image, no collective)",
                        "l2_protocol": f"inputs rotate over {R} independent copies ({R * ws_set / 1e6:.0f} MB >> L2 {l2 / 1e6:.0f} MB)",
-                       "backward": ("deterministic" if args.deterministic else "atomic") if cfg.backward else "none",
+                       "backward": args.backward if cfg.backward else "none",
                        "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
             "roofline": roof(dom),
             "roofline_all": {k: roof(k) for k in legs} | {"step": {"achieved": step_bytes / (step_ms * 1e-3) / 1e9,

@@ -56,8 +56,13 @@ typedef struct {
 /* Backward flags (bitmask). */
 enum {
   RAF_ACCUMULATE = 1,     /* add into the existing gradient pyramid instead of overwriting it      */
-  RAF_DETERMINISTIC = 2   /* bit-reproducible run to run (pull / sorted-segment variant, K3d)      */
+  RAF_DETERMINISTIC = 2,  /* REQUIRE the bit-reproducible pull variant (K3d); RAF_ERR_UNSUPPORTED
+                             if the layout is not eligible (needs channels-last, C % 4 == 0,
+                             sampling_ratio > 0, L*N <= 1500)                                       */
+  RAF_ATOMIC = 4          /* force the atomic scatter variant (zero-fill + red.global.add.v4.f32)  */
 };
+/* With neither RAF_DETERMINISTIC nor RAF_ATOMIC the library picks the pull variant when eligible
+ * and the atomic variant otherwise. */
 
 /* Bytes of device workspace the calls below need for these arguments (never 0; 256-aligned). */
 size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,

@@ -13,6 +13,7 @@ static std::atomic<uint64_t> g_launches{0};
 void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+constexpr int kBoffInts = 2048;  // boff[L*N + 1]; larger L*N falls back to the atomic backward
 static size_t esize(raf_dtype d) { return d == RAF_F32 ? 4 : 2; }
 
 static int check_levels(const raf_level* lv, int L) {
@@ -90,8 +91,8 @@ size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sam
                                      int flags) {
   (void)L; (void)out_h; (void)out_w; (void)sampling_ratio; (void)flags;
   const size_t k = K > 0 ? (size_t)K : 0;
-  // [levels K][perm K][counts 8] int32, each 256-aligned
-  return 256 + 2 * align256(4 * k) + 256;
+  // [bperm K][boff kBoffInts] int32 (pull backward), + slack; each region 256-aligned
+  return 256 + align256(4 * k) + align256(4 * kBoffInts) + 256;
 }
 
 int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
@@ -140,16 +141,38 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (rc) return rc;
   if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
-  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC)) return RAF_ERR_UNSUPPORTED;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
+  if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
   if (!gout_strides) return RAF_ERR_NULL;
   for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
   if (K > 0 && !grad_out) return RAF_ERR_NULL;
-  if (K > 0 && !ws) return RAF_ERR_NULL;
-  if (K > 0 && ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
+  if (!ws) return RAF_ERR_NULL;
+  if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
     return RAF_ERR_WORKSPACE;
-  if (flags & RAF_DETERMINISTIC) return RAF_ERR_UNSUPPORTED;  // K3d: not in this build yet
   cudaStream_t st = (cudaStream_t)stream;
+  LevelsParam p;
+  fill_param(grad_feats, L, &p);
+  const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
+  const bool cl = levels_vectorizable(grad_feats, L, 4, 4) &&
+                  (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype)));
 
+  // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
+  const bool pull_ok = cl && sampling_ratio > 0 && ws != nullptr &&
+                       (int64_t)L * grad_feats[0].n + 1 <= kBoffInts &&
+                       bucket_smem_bytes(L, grad_feats[0].n) <= 200 * 1024 &&
+                       ws_bytes >= roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags);
+  if (pull_ok && !(flags & RAF_ATOMIC)) {
+    int32_t* bperm = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + 256);
+    int32_t* boff = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(bperm) + align256(4 * (size_t)(K > 0 ? K : 0)));
+    rc = launch_bucket_rois(rois, K, L, grad_feats[0].n, finest_scale, bperm, boff, st);
+    if (rc) return rc;
+    rc = launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, bperm, boff,
+                              (flags & RAF_ACCUMULATE) ? 1 : 0, st);
+    if (rc != RAF_ERR_UNSUPPORTED) return rc;
+  }
+  if (flags & RAF_DETERMINISTIC) return RAF_ERR_UNSUPPORTED;
+
+  // ---- atomic variant (K3) -----------------------------------------------------------------------
   if (!(flags & RAF_ACCUMULATE)) {
     for (int l = 0; l < L; ++l) {
       const raf_level& v = grad_feats[l];
@@ -164,12 +187,6 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
     }
   }
   if (K == 0) return RAF_OK;
-
-  LevelsParam p;
-  fill_param(grad_feats, L, &p);
-  const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
-  const bool cl = levels_vectorizable(grad_feats, L, 4, 4) &&
-                  tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype));
   return launch_backward_atomic(p, gout_dtype, a, grad_out, gout_strides, cl, st);
 }
 

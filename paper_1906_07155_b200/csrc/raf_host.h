@@ -34,6 +34,17 @@ int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const R
                            const void* grad_out, const int64_t* gout_strides, bool channels_last,
                            cudaStream_t stream);
 
+// (level, image) stable bucketing for the pull backward: bperm[K], boff[L*N + 1].
+size_t bucket_smem_bytes(int L, int N);
+int launch_bucket_rois(const float* rois, int K, int L, int N, float finest_scale, int32_t* bperm,
+                       int32_t* boff, cudaStream_t stream);
+
+// Backward, deterministic pull formulation (channels-last, sampling_ratio > 0).  Writes every
+// gradient element exactly once (or adds into it when `accumulate`).
+int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
+                         const int64_t* gout_strides, const int32_t* bperm, const int32_t* boff, int accumulate,
+                         cudaStream_t stream);
+
 // Zero-fill of one strided level (used when the level is not one dense block).
 int launch_zero_level(float* data, int n, int c, int h, int w, int64_t sn, int64_t sc, int64_t sh,
                       int64_t sw, cudaStream_t stream);

@@ -72,6 +72,103 @@ assign_levels_kernel(const float* __restrict__ rois, int K, int L, float finest_
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Stable bucketing by (level, image): key = level * N + batch_idx.  Feeds the pull backward
+// (raf_backward_pull.cu), whose tiles walk the RoIs of their own (level, image) in ascending k --
+// a fixed order, hence bit-reproducible sums.  RoIs with an invalid batch index are dropped.
+//   bperm[K]      RoI indices grouped by key, ascending k inside a key
+//   boff[NK + 1]  start of every key's group (NK = L * N)
+// One CTA, 32 warps; warp w owns the contiguous RoI range [w*q, (w+1)*q).  cnt[w][key] first
+// counts, then (after a scan over keys, warps minor) holds the next free slot of (key, warp):
+// warp-private rows, so neither atomics nor block barriers inside the walks.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kLevelThreads, 1)
+bucket_rois_kernel(const float* __restrict__ rois, int K, int L, int N, float finest_scale,
+                   int32_t* __restrict__ bperm, int32_t* __restrict__ boff) {
+  extern __shared__ int s_cnt[];  // [32][NK + 1] then [NK + 1] totals/offsets
+  const int NK = L * N, NK1 = NK + 1;
+  int* s_tot = s_cnt + 32 * NK1;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int q = ((K + 31) / 32 + 31) & ~31;  // per-warp range, multiple of 32
+  const int lo = warp * q, hi = min(K, lo + q);
+  for (int i = tid; i < 32 * NK1 + NK1; i += kLevelThreads) s_cnt[i] = 0;
+  __syncthreads();
+
+  auto key_of = [&](int k) -> int {
+    if (k >= hi) return -1;
+    const float* r = rois + 5 * (int64_t)k;
+    const int b = batch_index_of(r[0], N);
+    if (b < 0) return NK;  // dropped
+    return level_of(r[1], r[2], r[3], r[4], L, finest_scale) * N + b;
+  };
+
+  int* mine = s_cnt + warp * NK1;
+  for (int k0 = lo; k0 < hi; k0 += 32) {
+    const int key = key_of(k0 + lane);
+    const unsigned peers = __match_any_sync(0xffffffffu, key);
+    if (key >= 0 && lane == __ffs(peers) - 1) mine[key] += __popc(peers);
+    __syncwarp();
+  }
+  __syncthreads();
+
+  // totals per key
+  for (int key = tid; key < NK1; key += kLevelThreads) {
+    int t = 0;
+    for (int w = 0; w < 32; ++w) t += s_cnt[w * NK1 + key];
+    s_tot[key] = t;
+  }
+  __syncthreads();
+  if (warp == 0) {  // exclusive scan of the totals over keys, 32 at a time
+    int carry = 0;
+    for (int base = 0; base < NK1; base += 32) {
+      const int key = base + lane;
+      const int v = key < NK1 ? s_tot[key] : 0;
+      int incl = v;
+      for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += o;
+      }
+      if (key < NK1) s_tot[key] = carry + incl - v;
+      carry += __shfl_sync(0xffffffffu, incl, 31);
+    }
+  }
+  __syncthreads();
+  for (int key = tid; key < NK1; key += kLevelThreads) {
+    if (key <= NK) boff[key] = s_tot[key];  // boff[NK] = number of kept RoIs
+    int run = s_tot[key];
+    for (int w = 0; w < 32; ++w) {
+      const int c = s_cnt[w * NK1 + key];
+      s_cnt[w * NK1 + key] = run;
+      run += c;
+    }
+  }
+  __syncthreads();
+
+  for (int k0 = lo; k0 < hi; k0 += 32) {
+    const int key = key_of(k0 + lane);
+    const unsigned peers = __match_any_sync(0xffffffffu, key);
+    const int base = (key >= 0) ? mine[key] : 0;
+    __syncwarp();
+    if (key >= 0 && key < NK) bperm[base + __popc(peers & ((1u << lane) - 1u))] = k0 + lane;
+    if (key >= 0 && lane == __ffs(peers) - 1) mine[key] = base + __popc(peers);
+    __syncwarp();
+  }
+}
+
+size_t bucket_smem_bytes(int L, int N) { return (size_t)33 * ((size_t)L * N + 1) * sizeof(int); }
+
+int launch_bucket_rois(const float* rois, int K, int L, int N, float finest_scale, int32_t* bperm,
+                       int32_t* boff, cudaStream_t stream) {
+  const size_t smem = bucket_smem_bytes(L, N);
+  if (smem > 200 * 1024) return RAF_ERR_UNSUPPORTED;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(bucket_rois_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return RAF_ERR_CUDA;
+  bucket_rois_kernel<<<1, kLevelThreads, smem, stream>>>(rois, K, L, N, finest_scale, bperm, boff);
+  count_launch();
+  return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;
+}
+
 int launch_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
                          int32_t* counts, int32_t* perm, cudaStream_t stream) {
   assign_levels_kernel<<<1, kLevelThreads, 0, stream>>>(rois, K, L, finest_scale, levels, counts,

@@ -169,42 +169,80 @@ def _bwd_case(wl, gout_dtype, layout, P=None, g=None, aligned=None, flags=0, ini
     return T.assert_backward_close(got, ref, S)
 
 
-@pytest.mark.parametrize("layout", ["cl", "nchw"])
-def test_backward_config1(layout):
-    _bwd_case(inputs.make_workload(1), "f32", layout)
+VARIANTS = [("cl", 0), ("cl", B.RAF_ATOMIC), ("cl", B.RAF_DETERMINISTIC), ("nchw", 0)]
 
 
-@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("layout,flags", VARIANTS)
+def test_backward_config1(layout, flags):
+    _bwd_case(inputs.make_workload(1), "f32", layout, flags=flags)
+
+
+@pytest.mark.parametrize("layout,flags", VARIANTS)
 @pytest.mark.parametrize("index,dtype,kw", [
     (2, "f32", dict(n_img=2, per_img=96, channels=64)),
+    (2, "f32", dict(n_img=1, per_img=300, channels=256)),   # > 256 RoIs in one bucket: two scan chunks
     (4, "bf16", dict(n_img=2, per_img=40, channels=32)),
     (5, "bf16", dict(n_img=3, per_img=64, channels=32)),
     (5, "f16", dict(n_img=2, per_img=50, channels=36)),
+    (5, "f32", dict(n_img=2, per_img=30, channels=1040)),   # more channel groups than threads per row
 ])
-def test_backward_reduced_configs(index, dtype, kw, layout):
-    _bwd_case(inputs.make_workload(index, **kw), dtype, layout)
+def test_backward_reduced_configs(index, dtype, kw, layout, flags):
+    _bwd_case(inputs.make_workload(index, **kw), dtype, layout, flags=flags)
 
 
-@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("layout,flags", [("cl", 0), ("cl", B.RAF_ATOMIC), ("nchw", 0)])
 @pytest.mark.parametrize("P,g,aligned", [((7, 7), 1, True), ((7, 7), 0, True), ((7, 7), 2, False),
-                                         ((5, 9), 3, True), ((14, 14), 2, True), ((7, 7), 0, False)])
-def test_backward_variants(P, g, aligned, layout):
+                                         ((5, 9), 3, True), ((14, 14), 2, True), ((7, 7), 0, False),
+                                         ((32, 32), 2, True), ((1, 1), 4, True), ((3, 2), 16, False)])
+def test_backward_variants(P, g, aligned, layout, flags):
     wl = inputs.make_workload(5, n_img=2, per_img=24, channels=8)
-    _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned)
+    _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned, flags=flags)
 
 
-@pytest.mark.parametrize("layout", ["cl", "nchw"])
-def test_backward_accumulate_mode(layout):
+def test_backward_degenerate_and_invalid_rois():
+    wl = inputs.make_workload(2, n_img=2, per_img=8, channels=16)
+    wl.rois = np.array([[0, 100, 100, 100, 100], [1, 300, 200, 100, 50], [0, -500, -500, -400, -400],
+                        [1, 0, 0, 1344, 800], [2, 10, 10, 90, 90], [-1, 10, 10, 90, 90],
+                        [0.5, 10, 10, 90, 90], [0, 1343.9, 799.9, 1344, 800], [1, 5000, 5000, 6000, 6000],
+                        [0, -3, -3, 2, 2], [1, 1340, 790, 1350, 810]], np.float32)
+    wl.grad_out = wl.grad_out[:len(wl.rois)]
+    for layout, flags in VARIANTS:
+        cfg = wl.cfg
+        got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, layout,
+                                       "f32", flags)
+        ref, S = R.backward(cfg.level_shapes, cfg.scales, go_exact, wl.rois, (7, 7), 2, True, 56.0)
+        T.assert_backward_close(got, ref, S)
+
+
+def test_deterministic_backward_is_bit_reproducible():
+    wl = inputs.make_workload(5, n_img=3, per_img=200, channels=64)
+    cfg = wl.cfg
+    runs = [T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl", "bf16",
+                           B.RAF_DETERMINISTIC)[0] for _ in range(3)]
+    for other in runs[1:]:
+        for a, b in zip(runs[0], other):
+            assert np.array_equal(a, b)
+    # requesting determinism for an ineligible layout is refused, not silently downgraded
+    with pytest.raises(B.RafError) as e:
+        T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "nchw", "f32",
+                       B.RAF_DETERMINISTIC)
+    assert e.value.status == -5
+
+
+@pytest.mark.parametrize("layout,flags", VARIANTS)
+def test_backward_accumulate_mode(layout, flags):
     wl = inputs.make_workload(2, n_img=2, per_img=32, channels=16)
     rng = np.random.default_rng(3)
     init = [rng.standard_normal(s).astype(np.float32).astype(np.float64) for s in wl.cfg.level_shapes]
-    _bwd_case(wl, "f32", layout, flags=B.RAF_ACCUMULATE, init=init)
+    _bwd_case(wl, "f32", layout, flags=flags | B.RAF_ACCUMULATE, init=init)
 
 
-def test_backward_full_size_config2():
+@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC])
+def test_backward_full_size_config2(flags):
     wl = inputs.make_workload(2, with_feats=False)
     cfg = wl.cfg
-    got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl")
+    got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl",
+                                   "f32", flags)
     # the oracle on a channel slice (channels are independent)
     sl = slice(40, 56)
     shapes = [(s[0], 16, s[2], s[3]) for s in cfg.level_shapes]

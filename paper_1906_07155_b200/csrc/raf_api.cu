@@ -87,12 +87,28 @@ using namespace raf;
 
 extern "C" {
 
+// Workspace carve-up (pull backward): [bperm K int32][boff kBoffInts int32][bwin K int4][taps].
+struct WsLayout {
+  size_t bperm, boff, bwin, taps, total;
+};
+static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
+  const size_t k = K > 0 ? (size_t)K : 0;
+  const size_t g = sampling_ratio > 0 ? (size_t)sampling_ratio : 0;
+  WsLayout w;
+  w.bperm = 256;
+  w.boff = w.bperm + align256(4 * k);
+  w.bwin = w.boff + align256(4 * (size_t)kBoffInts);
+  w.taps = w.bwin + align256(16 * k);
+  w.total = w.taps + align256(k * (size_t)(out_h + out_w) * 2 * g * sizeof(PullTap)) + 256;
+  return w;
+}
+
 size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,
                                      int flags) {
-  (void)L; (void)out_h; (void)out_w; (void)sampling_ratio; (void)flags;
-  const size_t k = K > 0 ? (size_t)K : 0;
-  // [bperm K][boff kBoffInts] int32 (pull backward), + slack; each region 256-aligned
-  return 256 + align256(4 * k) + align256(4 * kBoffInts) + 256;
+  (void)L; (void)flags;
+  if (out_h < 1) out_h = 1;
+  if (out_w < 1) out_w = 1;
+  return ws_layout(K, out_h, out_w, sampling_ratio).total;
 }
 
 int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
@@ -157,16 +173,22 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                   (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype)));
 
   // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
-  const bool pull_ok = cl && sampling_ratio > 0 && ws != nullptr &&
-                       (int64_t)L * grad_feats[0].n + 1 <= kBoffInts &&
-                       bucket_smem_bytes(L, grad_feats[0].n) <= 200 * 1024 &&
-                       ws_bytes >= roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags);
+  bool pull_ok = cl && sampling_ratio > 0 && (int64_t)L * grad_feats[0].n + 1 <= kBoffInts &&
+                 bucket_smem_bytes(L, grad_feats[0].n) <= 200 * 1024;
+  for (int l = 0; l < L; ++l)   // tap tables keep pixel indices in 24 bits
+    if (grad_feats[l].h >= 0xffffff || grad_feats[l].w >= 0xffffff) pull_ok = false;
   if (pull_ok && !(flags & RAF_ATOMIC)) {
-    int32_t* bperm = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(ws) + 256);
-    int32_t* boff = reinterpret_cast<int32_t*>(reinterpret_cast<char*>(bperm) + align256(4 * (size_t)(K > 0 ? K : 0)));
-    rc = launch_bucket_rois(rois, K, L, grad_feats[0].n, finest_scale, bperm, boff, st);
+    const WsLayout w = ws_layout(K, out_h, out_w, sampling_ratio);
+    char* base = reinterpret_cast<char*>(ws);
+    int32_t* bperm = reinterpret_cast<int32_t*>(base + w.bperm);
+    int32_t* boff = reinterpret_cast<int32_t*>(base + w.boff);
+    int4* bwin = reinterpret_cast<int4*>(base + w.bwin);
+    PullTap* taps = reinterpret_cast<PullTap*>(base + w.taps);
+    rc = launch_bucket_rois(p, a, bperm, boff, bwin, st);
     if (rc) return rc;
-    rc = launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, bperm, boff,
+    rc = launch_pull_taps(p, a, taps, st);
+    if (rc) return rc;
+    rc = launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, bperm, boff, bwin, taps,
                               (flags & RAF_ACCUMULATE) ? 1 : 0, st);
     if (rc != RAF_ERR_UNSUPPORTED) return rc;
   }

@@ -34,16 +34,26 @@ int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const R
                            const void* grad_out, const int64_t* gout_strides, bool channels_last,
                            cudaStream_t stream);
 
-// (level, image) stable bucketing for the pull backward: bperm[K], boff[L*N + 1].
+// (level, image) stable bucketing for the pull backward: bperm[K], boff[L*N + 1], and (optional)
+// bwin[K] = conservative touched-pixel window of every kept RoI, in bperm order.
 size_t bucket_smem_bytes(int L, int N);
-int launch_bucket_rois(const float* rois, int K, int L, int N, float finest_scale, int32_t* bperm,
-                       int32_t* boff, cudaStream_t stream);
+int launch_bucket_rois(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, int32_t* boff, int4* bwin,
+                       cudaStream_t stream);
+
+// One merged bilinear tap of an output bin along one axis (pull backward tap tables).
+struct PullTap {
+  uint32_t pb;  // pixel | bin << 24; pixel == 0xffffff marks an empty slot
+  float w;      // weight (y taps carry 1/count)
+};
+
+// Tap tables taps[K][PH + PW][2 * sampling_ratio] for the pull backward (sampling_ratio > 0).
+int launch_pull_taps(const LevelsParam& lv, const RoiArgs& a, PullTap* taps, cudaStream_t stream);
 
 // Backward, deterministic pull formulation (channels-last, sampling_ratio > 0).  Writes every
 // gradient element exactly once (or adds into it when `accumulate`).
 int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
-                         const int64_t* gout_strides, const int32_t* bperm, const int32_t* boff, int accumulate,
-                         cudaStream_t stream);
+                         const int64_t* gout_strides, const int32_t* bperm, const int32_t* boff,
+                         const int4* bwin, const PullTap* taps, int accumulate, cudaStream_t stream);
 
 // Zero-fill of one strided level (used when the level is not one dense block).
 int launch_zero_level(float* data, int n, int c, int h, int w, int64_t sn, int64_t sc, int64_t sh,

@@ -121,23 +121,31 @@ __device__ __forceinline__ void fma4(float4& acc, float w, const float4& v) {
   acc.z = fmaf(w, v.z, acc.z); acc.w = fmaf(w, v.w, acc.w);
 }
 
-constexpr int kNC = 64;      // candidates per build/consume pass
+constexpr int kNC = 64;            // candidates per build/consume pass
 constexpr int kMaxTapChunks = 4;   // <= 128 taps per axis (eligibility checked on the host)
+constexpr uint32_t kOffMask = 0x00ffffffu;
 
-struct PullInfo {   // first entry of a (candidate, row) or (candidate, column) + entry count
-  uint32_t meta;    // bin | count << 8
-  float w;
+// Up to two entries of a (candidate, row) or (candidate, column): element offset into grad_out
+// (bin * stride, premultiplied, 24 bits) and weight; the total entry count sits in m0's top byte.
+// More than two entries (bins narrower than half a pixel) are served from the ballot masks.
+struct __align__(16) PullInfo {
+  uint32_t m0;   // off0 | count << 24
+  float w0;
+  uint32_t off1;
+  float w1;
 };
 
-template <typename T>
+template <typename T, bool kFull>
 __global__ void __launch_bounds__(kPullThreads, 4)
-bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gout, int64_t gs_k,
-                int64_t gs_h, int64_t gs_w, const int32_t* __restrict__ bperm,
+bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gout, int gs_k,
+                int gs_h, int gs_w, const int32_t* __restrict__ bperm,
                 const int32_t* __restrict__ boff, const int4* __restrict__ bwin,
                 const PullTap* __restrict__ taps, const PullTiles tiles, int accumulate) {
   __shared__ int s_k[kPullThreads];
   __shared__ int s_wcount[kPullThreads / 32];
-  __shared__ __align__(16) PullInfo s_info[kNC][16];   // [c][0..7] rows, [c][8..15] columns
+  __shared__ int s_goff[kNC];                          // k * gs_k
+  __shared__ PullInfo s_info[kNC][16];                 // [c][0..7] rows, [c][8..15] columns
+  __shared__ unsigned char s_cnt[16][kNC];             // entry counts, transposed (ballot-friendly)
   extern __shared__ uint32_t s_mask[];                 // [kNC][16][nq]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -145,32 +153,28 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
   const int nty = a.PH * slots, ntx = a.PW * slots;
   const int nq = (max(nty, ntx) + 31) >> 5;
 
-  // ---- decode the tile --------------------------------------------------------------------------
+  // ---- decode the tile: blockIdx.y = tile within the pyramid (coarsest level first),
+  //      blockIdx.x = image * chunks + chunk (fastest, so heavy tiles of all images start first)
   int pos = 0;
-  while (pos + 1 < lv.L && (int)blockIdx.x >= tiles.start[pos + 1]) ++pos;
+  while (pos + 1 < lv.L && (int)blockIdx.y >= tiles.start[pos + 1]) ++pos;
   const int level = tiles.order[pos];
-  int rem = blockIdx.x - tiles.start[pos];
-  const int chunk = rem % tiles.chunks; rem /= tiles.chunks;
-  const int txi = rem % tiles.tiles_x[level]; rem /= tiles.tiles_x[level];
-  const int tyi = rem % tiles.tiles_y[level];
-  const int n = rem / tiles.tiles_y[level];
+  const int trem = blockIdx.y - tiles.start[pos];
+  const int tyi = trem / tiles.tiles_x[level], txi = trem - tyi * tiles.tiles_x[level];
+  const int n = blockIdx.x / tiles.chunks, chunk = blockIdx.x - n * tiles.chunks;
   const int H = lv.h[level], W = lv.w[level];
   const int y0 = tyi * kTH, x0 = txi * kTW;
   const int y1 = min(y0 + kTH, H) - 1, x1 = min(x0 + kTW, W) - 1;  // inclusive
 
   const int y = y0 + warp;               // this warp's pixel row
   const bool row_live = y <= y1;
-  int chA, chB;
-  Gout8<T>::channels(lane, chA, chB);
-  chA += chunk * Gout8<T>::kChunk;
-  chB += chunk * Gout8<T>::kChunk;
-  const bool actA = chA < lv.c, actB = chB < lv.c;
+  const int chA = chunk * 256 + lane * 4, chB = chA + 128;
+  const bool actA = kFull || chA < lv.c, actB = kFull || chB < lv.c;
   // inactive lanes read channel 0 (valid memory) and never store: no predicates in the hot loop
   const T* goutA = gout + (actA ? chA : 0);
-  const int dAB = (actB ? chB : 0) - (actA ? chA : 0);
+  const int dAB = kFull ? 128 : (actB ? chB : 0) - (actA ? chA : 0);
+  const int sw = (int)lv.sw[level];
   float* grow = reinterpret_cast<float*>(const_cast<void*>(lv.data[level])) + (int64_t)n * lv.sn[level] +
-                (int64_t)y * lv.sh[level] + (int64_t)x0 * lv.sw[level];
-  const int64_t sw = lv.sw[level];
+                (int64_t)y * lv.sh[level] + (int64_t)x0 * sw + chA;
   const int npx = x1 - x0 + 1;
 
   const int key = level * lv.n + n;
@@ -201,9 +205,10 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
       const int nc = min(kNC, ncand - p0);
       // ---- (B) tables of this pass: warp per candidate, lanes = taps ---------------------------
       for (int c = warp; c < nc; c += kPullThreads / 32) {
-        const PullTap* ty = taps + (int64_t)s_k[p0 + c] * (nty + ntx);
+        const int k = s_k[p0 + c];
+        const PullTap* ty = taps + (int64_t)k * (nty + ntx);
         const PullTap* tx = ty + nty;
-        int cnt = 0, first = -1;       // lanes 0..7: row `lane`; lanes 8..15: column `lane - 8`
+        int cnt = 0, e0 = -1, e1 = -1;   // lanes 0..7: row `lane`; lanes 8..15: column `lane - 8`
         for (int q = 0; q < nq; ++q) {
           const int t = q * 32 + lane;
           const int rely = (t < nty) ? (int)(__ldg(&ty[t].pb) & kPixMask) - y0 : -1;
@@ -218,83 +223,109 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
           }
           if (lane < 16) {
             s_mask[(c * 16 + lane) * nq + q] = mine;
-            if (first < 0 && mine) first = q * 32 + __ffs(mine) - 1;
             cnt += __popc(mine);
+            if (e0 < 0 && mine) { e0 = q * 32 + __ffs(mine) - 1; mine &= mine - 1; }
+            if (e1 < 0 && mine) e1 = q * 32 + __ffs(mine) - 1;
           }
         }
         if (lane < 16) {
+          const PullTap* tb = lane < 8 ? ty : tx;
+          const uint32_t stride = (uint32_t)(lane < 8 ? gs_h : gs_w);
           PullInfo inf;
-          inf.meta = 0; inf.w = 0.0f;
-          if (cnt) {
-            const PullTap e = (lane < 8 ? ty : tx)[first];
-            inf.meta = (e.pb >> 24) | ((uint32_t)cnt << 8);
-            inf.w = e.w;
+          inf.m0 = 0; inf.w0 = 0.0f; inf.off1 = 0; inf.w1 = 0.0f;
+          if (e0 >= 0) {
+            const PullTap e = tb[e0];
+            inf.m0 = ((e.pb >> 24) * stride) | ((uint32_t)min(cnt, 255) << 24);
+            inf.w0 = e.w;
+          }
+          if (e1 >= 0) {
+            const PullTap e = tb[e1];
+            inf.off1 = (e.pb >> 24) * stride;
+            inf.w1 = e.w;
           }
           s_info[c][lane] = inf;
+          s_cnt[lane][c] = (unsigned char)min(cnt, 255);
         }
+        if (lane == 0) s_goff[c] = k * gs_k;
       }
       __syncthreads();
 
       // ---- (C) consume: warp = pixel row, one pixel at a time, lanes = channels ----------------
       if (row_live) {
-        for (int j = 0; j < npx; ++j) {
-          float* gp = grow + (int64_t)j * sw;
+        // candidates with an entry on this row (bit c of rm0 / bit c-32 of rm1)
+        const unsigned rm0 = __ballot_sync(0xffffffffu, lane < nc && s_cnt[warp][lane] != 0);
+        const unsigned rm1 = __ballot_sync(0xffffffffu, 32 + lane < nc && s_cnt[warp][32 + lane] != 0);
+        float* gp = grow;
+        for (int j = 0; j < npx; ++j, gp += sw) {
           float4 accA = make_float4(0.f, 0.f, 0.f, 0.f), accB = accA;
           if (accumulate || npass) {
-            if (actA) accA = *reinterpret_cast<const float4*>(gp + chA);
-            if (actB) accB = *reinterpret_cast<const float4*>(gp + chB);
+            if (actA) accA = *reinterpret_cast<const float4*>(gp);
+            if (actB) accB = *reinterpret_cast<const float4*>(gp + 128);
           }
-          for (int c = 0; c < nc; ++c) {
-            const PullInfo iy = s_info[c][warp];
-            if (iy.meta == 0) continue;
-            const PullInfo ix = s_info[c][8 + j];
-            if (ix.meta == 0) continue;
-            const int k = s_k[p0 + c];
-            const T* gk = goutA + (int64_t)k * gs_k;
-            const PullTap* ty = taps + (int64_t)k * (nty + ntx);
-            const PullTap* tx = ty + nty;
-            const int nyE = iy.meta >> 8, nxE = ix.meta >> 8;
-            // all x entries of this column against one y entry (ph, wy)
-            auto row_entry = [&](int ph, float wy) {
-              const T* gy = gk + (int64_t)ph * gs_h;
-              {
-                const T* p = gy + (int64_t)(ix.meta & 0xffu) * gs_w;
-                const float w = wy * ix.w;
-                fma4(accA, w, ldg4<T>(p));
-                fma4(accB, w, ldg4<T>(p + dAB));
-              }
-              if (nxE > 1) {
-                bool skip = true;                       // the first entry is already done
-                for (int q = 0; q < nq; ++q) {
-                  unsigned mm = s_mask[(c * 16 + 8 + j) * nq + q];
-                  if (skip && mm) { mm &= mm - 1; skip = false; }
-                  while (mm) {
-                    const PullTap e = tx[q * 32 + __ffs(mm) - 1];
-                    mm &= mm - 1;
-                    const T* p = gy + (int64_t)(e.pb >> 24) * gs_w;
-                    const float w = wy * e.w;
-                    fma4(accA, w, ldg4<T>(p));
-                    fma4(accB, w, ldg4<T>(p + dAB));
+          unsigned cm[2];
+          cm[0] = rm0 & __ballot_sync(0xffffffffu, s_cnt[8 + j][lane] != 0);
+          cm[1] = rm1 & __ballot_sync(0xffffffffu, s_cnt[8 + j][32 + lane] != 0);
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            unsigned mm = cm[half];
+            while (mm) {
+              const int c = half * 32 + __ffs(mm) - 1;
+              mm &= mm - 1;
+              const PullInfo iy = s_info[c][warp];
+              const PullInfo ix = s_info[c][8 + j];
+              const T* gk = goutA + s_goff[c];
+              const uint32_t cy = iy.m0 >> 24, cx = ix.m0 >> 24;
+              if (cy <= 2 && cx <= 2) {
+                const uint32_t oy0 = iy.m0 & kOffMask, ox0 = ix.m0 & kOffMask;
+                {
+                  const T* p = gk + (oy0 + ox0);
+                  const float w = iy.w0 * ix.w0;
+                  fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
+                }
+                if (cx == 2) {
+                  const T* p = gk + (oy0 + ix.off1);
+                  const float w = iy.w0 * ix.w1;
+                  fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
+                }
+                if (cy == 2) {
+                  {
+                    const T* p = gk + (iy.off1 + ox0);
+                    const float w = iy.w1 * ix.w0;
+                    fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
+                  }
+                  if (cx == 2) {
+                    const T* p = gk + (iy.off1 + ix.off1);
+                    const float w = iy.w1 * ix.w1;
+                    fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
                   }
                 }
-              }
-            };
-            row_entry((int)(iy.meta & 0xffu), iy.w);
-            if (nyE > 1) {
-              bool skip = true;
-              for (int q = 0; q < nq; ++q) {
-                unsigned mm = s_mask[(c * 16 + warp) * nq + q];
-                if (skip && mm) { mm &= mm - 1; skip = false; }
-                while (mm) {
-                  const PullTap e = ty[q * 32 + __ffs(mm) - 1];
-                  mm &= mm - 1;
-                  row_entry((int)(e.pb >> 24), e.w);
+              } else {   // rare: more than two entries on an axis -> walk the ballot masks
+                const int k = s_k[p0 + c];
+                const PullTap* ty = taps + (int64_t)k * (nty + ntx);
+                const PullTap* tx = ty + nty;
+                for (int qy = 0; qy < nq; ++qy) {
+                  unsigned my = s_mask[(c * 16 + warp) * nq + qy];
+                  while (my) {
+                    const PullTap ey = ty[qy * 32 + __ffs(my) - 1];
+                    my &= my - 1;
+                    const T* gy = gk + (ey.pb >> 24) * (uint32_t)gs_h;
+                    for (int qx = 0; qx < nq; ++qx) {
+                      unsigned mx = s_mask[(c * 16 + 8 + j) * nq + qx];
+                      while (mx) {
+                        const PullTap ex = tx[qx * 32 + __ffs(mx) - 1];
+                        mx &= mx - 1;
+                        const T* p = gy + (ex.pb >> 24) * (uint32_t)gs_w;
+                        const float w = ey.w * ex.w;
+                        fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
+                      }
+                    }
+                  }
                 }
               }
             }
           }
-          if (actA) *reinterpret_cast<float4*>(gp + chA) = accA;
-          if (actB) *reinterpret_cast<float4*>(gp + chB) = accB;
+          if (actA) *reinterpret_cast<float4*>(gp) = accA;
+          if (actB) *reinterpret_cast<float4*>(gp + 128) = accB;
         }
       }
       ++npass;
@@ -304,10 +335,10 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
 
   if (npass == 0 && !accumulate && row_live) {   // nothing lands in this tile: zeros
     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int j = 0; j < npx; ++j) {
-      float* gp = grow + (int64_t)j * sw;
-      if (actA) *reinterpret_cast<float4*>(gp + chA) = z;
-      if (actB) *reinterpret_cast<float4*>(gp + chB) = z;
+    float* gp = grow;
+    for (int j = 0; j < npx; ++j, gp += sw) {
+      if (actA) *reinterpret_cast<float4*>(gp) = z;
+      if (actB) *reinterpret_cast<float4*>(gp + 128) = z;
     }
   }
 }
@@ -317,7 +348,7 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
                       const int32_t* bperm, const int32_t* boff, const int4* bwin, const PullTap* taps,
                       int accumulate, cudaStream_t stream) {
   PullTiles t;
-  t.chunks = (lv.c + Gout8<T>::kChunk - 1) / Gout8<T>::kChunk;
+  t.chunks = (lv.c + 255) / 256;
   int64_t total = 0;
   for (int i = 0; i < lv.L; ++i) {
     const int l = lv.L - 1 - i;  // coarsest level first
@@ -325,17 +356,28 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
     t.tiles_y[l] = (lv.h[l] + kTH - 1) / kTH;
     t.tiles_x[l] = (lv.w[l] + kTW - 1) / kTW;
     t.start[i] = (int32_t)total;
-    total += (int64_t)lv.n * t.tiles_y[l] * t.tiles_x[l] * t.chunks;
+    total += (int64_t)t.tiles_y[l] * t.tiles_x[l];
   }
-  if (total >= ((int64_t)1 << 31)) return RAF_ERR_UNSUPPORTED;
   t.start[lv.L] = (int32_t)total;
+  const int64_t gy = (int64_t)lv.n * t.chunks;
   const int ntaps = 2 * a.sampling_ratio * (a.PH > a.PW ? a.PH : a.PW);
   const int nq = (ntaps + 31) / 32;
-  if (nq > kMaxTapChunks) return RAF_ERR_UNSUPPORTED;
+  // 32-bit / 24-bit offset arithmetic inside the kernel: grad_out must fit
+  const int64_t span = (int64_t)a.K * gs[0] + (int64_t)a.PH * gs[2] + (int64_t)a.PW * gs[3] + lv.c;
+  if (total > 65535 || gy >= ((int64_t)1 << 31) || nq > kMaxTapChunks || span >= ((int64_t)1 << 31) ||
+      (int64_t)a.PH * gs[2] >= (1 << 24) || (int64_t)a.PW * gs[3] >= (1 << 24))
+    return RAF_ERR_UNSUPPORTED;
+  for (int l = 0; l < lv.L; ++l)
+    if ((int64_t)lv.w[l] * lv.sw[l] >= ((int64_t)1 << 31)) return RAF_ERR_UNSUPPORTED;
   const size_t smem = sizeof(uint32_t) * kNC * 16 * nq;
-  bwd_pull_kernel<T><<<(unsigned)total, kPullThreads, smem, stream>>>(lv, a, reinterpret_cast<const T*>(gout), gs[0],
-                                                                      gs[2], gs[3], bperm, boff, bwin, taps, t,
-                                                                      accumulate);
+  const dim3 grid((unsigned)gy, (unsigned)total);
+  const T* g = reinterpret_cast<const T*>(gout);
+  if (lv.c % 256 == 0)
+    bwd_pull_kernel<T, true><<<grid, kPullThreads, smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], bperm,
+                                                                   boff, bwin, taps, t, accumulate);
+  else
+    bwd_pull_kernel<T, false><<<grid, kPullThreads, smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], bperm,
+                                                                    boff, bwin, taps, t, accumulate);
   count_launch();
   return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;
 }

@@ -42,6 +42,8 @@ struct PullTiles {
   int32_t order[kMaxLevels];      // level processed at position i (coarsest first)
   int32_t start[kMaxLevels + 1];  // first block of position i
   int32_t tiles_y[kMaxLevels], tiles_x[kMaxLevels];
+  int32_t th[kMaxLevels];         // tile rows of the level (1, 2, 4 or 8): small (dense) levels get
+                                  // short tiles = more CTAs per RoI-heavy area, shorter critical path
   int32_t chunks;                 // channel chunks of 256
 };
 
@@ -162,20 +164,19 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
   const int tyi = trem / tiles.tiles_x[level], txi = trem - tyi * tiles.tiles_x[level];
   const int n = blockIdx.x / tiles.chunks, chunk = blockIdx.x - n * tiles.chunks;
   const int H = lv.h[level], W = lv.w[level];
-  const int y0 = tyi * kTH, x0 = txi * kTW;
-  const int y1 = min(y0 + kTH, H) - 1, x1 = min(x0 + kTW, W) - 1;  // inclusive
-
-  const int y = y0 + warp;               // this warp's pixel row
-  const bool row_live = y <= y1;
+  const int TH = tiles.th[level];
+  const int y0 = tyi * TH, x0 = txi * kTW;
+  const int y1 = min(y0 + TH, H) - 1, x1 = min(x0 + kTW, W) - 1;  // inclusive
   const int chA = chunk * 256 + lane * 4, chB = chA + 128;
   const bool actA = kFull || chA < lv.c, actB = kFull || chB < lv.c;
   // inactive lanes read channel 0 (valid memory) and never store: no predicates in the hot loop
   const T* goutA = gout + (actA ? chA : 0);
   const int dAB = kFull ? 128 : (actB ? chB : 0) - (actA ? chA : 0);
   const int sw = (int)lv.sw[level];
-  float* grow = reinterpret_cast<float*>(const_cast<void*>(lv.data[level])) + (int64_t)n * lv.sn[level] +
-                (int64_t)y * lv.sh[level] + (int64_t)x0 * sw + chA;
-  const int npx = x1 - x0 + 1;
+  const int sh = (int)lv.sh[level];
+  float* gtile = reinterpret_cast<float*>(const_cast<void*>(lv.data[level])) + (int64_t)n * lv.sn[level] +
+                 (int64_t)y0 * sh + (int64_t)x0 * sw + chA;
+  const int npx = x1 - x0 + 1, npy = y1 - y0 + 1;
 
   const int key = level * lv.n + n;
   const int bbeg = boff[key], bend = boff[key + 1];
@@ -250,28 +251,29 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
       }
       __syncthreads();
 
-      // ---- (C) consume: warp = pixel row, one pixel at a time, lanes = channels ----------------
-      if (row_live) {
-        // candidates with an entry on this row (bit c of rm0 / bit c-32 of rm1)
-        const unsigned rm0 = __ballot_sync(0xffffffffu, lane < nc && s_cnt[warp][lane] != 0);
-        const unsigned rm1 = __ballot_sync(0xffffffffu, 32 + lane < nc && s_cnt[warp][32 + lane] != 0);
-        float* gp = grow;
-        for (int j = 0; j < npx; ++j, gp += sw) {
+      // ---- (C) consume: warp w takes pixel (row i, column (w + i) % 8) for every tile row i: one
+      //      pixel of every row and (for 8-row tiles) of every column, so the warps of a CTA carry
+      //      about the same load; one pixel at a time, lanes = channels -------------------------
+      for (int i = 0; i < npy; ++i) {
+        const int j = (warp + i) & 7;
+        if (j >= npx) continue;
+        {
+          float* gp = gtile + i * sh + j * sw;
           float4 accA = make_float4(0.f, 0.f, 0.f, 0.f), accB = accA;
           if (accumulate || npass) {
             if (actA) accA = *reinterpret_cast<const float4*>(gp);
             if (actB) accB = *reinterpret_cast<const float4*>(gp + 128);
           }
           unsigned cm[2];
-          cm[0] = rm0 & __ballot_sync(0xffffffffu, s_cnt[8 + j][lane] != 0);
-          cm[1] = rm1 & __ballot_sync(0xffffffffu, s_cnt[8 + j][32 + lane] != 0);
+          cm[0] = __ballot_sync(0xffffffffu, lane < nc && s_cnt[i][lane] != 0 && s_cnt[8 + j][lane] != 0);
+          cm[1] = __ballot_sync(0xffffffffu, 32 + lane < nc && s_cnt[i][32 + lane] != 0 && s_cnt[8 + j][32 + lane] != 0);
 #pragma unroll
           for (int half = 0; half < 2; ++half) {
             unsigned mm = cm[half];
             while (mm) {
               const int c = half * 32 + __ffs(mm) - 1;
               mm &= mm - 1;
-              const PullInfo iy = s_info[c][warp];
+              const PullInfo iy = s_info[c][i];
               const PullInfo ix = s_info[c][8 + j];
               const T* gk = goutA + s_goff[c];
               const uint32_t cy = iy.m0 >> 24, cx = ix.m0 >> 24;
@@ -304,7 +306,7 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
                 const PullTap* ty = taps + (int64_t)k * (nty + ntx);
                 const PullTap* tx = ty + nty;
                 for (int qy = 0; qy < nq; ++qy) {
-                  unsigned my = s_mask[(c * 16 + warp) * nq + qy];
+                  unsigned my = s_mask[(c * 16 + i) * nq + qy];
                   while (my) {
                     const PullTap ey = ty[qy * 32 + __ffs(my) - 1];
                     my &= my - 1;
@@ -329,14 +331,17 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
         }
       }
       ++npass;
-      __syncthreads();    // tables and s_k are rewritten by the next pass / scan chunk
+      if (p0 + kNC < ncand || s0 + kPullThreads < bend)
+        __syncthreads();  // tables and s_k are rewritten by the next pass / scan chunk
     }
   }
 
-  if (npass == 0 && !accumulate && row_live) {   // nothing lands in this tile: zeros
+  if (npass == 0 && !accumulate) {   // nothing lands in this tile: zeros
     const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
-    float* gp = grow;
-    for (int j = 0; j < npx; ++j, gp += sw) {
+    for (int i = 0; i < npy; ++i) {
+      const int j = (warp + i) & 7;
+      if (j >= npx) continue;
+      float* gp = gtile + i * sh + j * sw;
       if (actA) *reinterpret_cast<float4*>(gp) = z;
       if (actB) *reinterpret_cast<float4*>(gp + 128) = z;
     }
@@ -353,7 +358,10 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
   for (int i = 0; i < lv.L; ++i) {
     const int l = lv.L - 1 - i;  // coarsest level first
     t.order[i] = l;
-    t.tiles_y[l] = (lv.h[l] + kTH - 1) / kTH;
+    int th = kTH;                // aim for >= 128 tiles per level and image
+    while (th > 1 && (int64_t)lv.h[l] * lv.w[l] < (int64_t)128 * th * kTW) th >>= 1;
+    t.th[l] = th;
+    t.tiles_y[l] = (lv.h[l] + th - 1) / th;
     t.tiles_x[l] = (lv.w[l] + kTW - 1) / kTW;
     t.start[i] = (int32_t)total;
     total += (int64_t)t.tiles_y[l] * t.tiles_x[l];
@@ -368,7 +376,7 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
       (int64_t)a.PH * gs[2] >= (1 << 24) || (int64_t)a.PW * gs[3] >= (1 << 24))
     return RAF_ERR_UNSUPPORTED;
   for (int l = 0; l < lv.L; ++l)
-    if ((int64_t)lv.w[l] * lv.sw[l] >= ((int64_t)1 << 31)) return RAF_ERR_UNSUPPORTED;
+    if ((int64_t)lv.w[l] * lv.sw[l] + (int64_t)kTH * lv.sh[l] >= ((int64_t)1 << 31)) return RAF_ERR_UNSUPPORTED;
   const size_t smem = sizeof(uint32_t) * kNC * 16 * nq;
   const dim3 grid((unsigned)gy, (unsigned)total);
   const T* g = reinterpret_cast<const T*>(gout);

@@ -184,9 +184,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
     int32_t* boff = reinterpret_cast<int32_t*>(base + w.boff);
     int4* bwin = reinterpret_cast<int4*>(base + w.bwin);
     PullTap* taps = reinterpret_cast<PullTap*>(base + w.taps);
-    rc = launch_bucket_rois(p, a, bperm, boff, bwin, st);
-    if (rc) return rc;
-    rc = launch_pull_taps(p, a, taps, st);
+    rc = launch_pull_prep(p, a, bperm, boff, bwin, taps, st);
     if (rc) return rc;
     rc = launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, bperm, boff, bwin, taps,
                               (flags & RAF_ACCUMULATE) ? 1 : 0, st);

@@ -34,20 +34,18 @@ int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const R
                            const void* grad_out, const int64_t* gout_strides, bool channels_last,
                            cudaStream_t stream);
 
-// (level, image) stable bucketing for the pull backward: bperm[K], boff[L*N + 1], and (optional)
-// bwin[K] = conservative touched-pixel window of every kept RoI, in bperm order.
-size_t bucket_smem_bytes(int L, int N);
-int launch_bucket_rois(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, int32_t* boff, int4* bwin,
-                       cudaStream_t stream);
-
 // One merged bilinear tap of an output bin along one axis (pull backward tap tables).
 struct PullTap {
   uint32_t pb;  // pixel | bin << 24; pixel == 0xffffff marks an empty slot
   float w;      // weight (y taps carry 1/count)
 };
 
-// Tap tables taps[K][PH + PW][2 * sampling_ratio] for the pull backward (sampling_ratio > 0).
-int launch_pull_taps(const LevelsParam& lv, const RoiArgs& a, PullTap* taps, cudaStream_t stream);
+// Prep launch of the pull backward (sampling_ratio > 0): block 0 buckets the RoIs by (level, image)
+// -- bperm[K], boff[L*N + 1], bwin[K] = conservative touched-pixel window of every kept RoI in
+// bperm order -- and the other blocks write the tap tables taps[K][PH + PW][2 * sampling_ratio].
+size_t bucket_smem_bytes(int L, int N);
+int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, int32_t* boff, int4* bwin,
+                     PullTap* taps, cudaStream_t stream);
 
 // Backward, deterministic pull formulation (channels-last, sampling_ratio > 0).  Writes every
 // gradient element exactly once (or adds into it when `accumulate`).

@@ -3,101 +3,200 @@
 //   out[k,c,ph,pw] = (1/count) * sum_{iy,ix} bilinear(F_{level_k}[b_k,c], y(ph,iy), x(pw,ix))
 //
 // Two kernels:
-//  * fwd_cl_kernel   channels-last fast path: one CTA per RoI.  The RoI's level, image and its
-//                    per-axis sample tables (pixel offsets + bilinear weights, computed ONCE per
-//                    sample and reused by every channel -- north_star) are staged in shared memory;
-//                    then threads are laid out (channel-vector, bin): each 128-bit load covers 4
-//                    fp32 / 8 half channels of one tap, a warp reads 512 contiguous bytes.
+//  * fwd_cl_kernel   channels-last fast path: one CTA per (RoI, 32 channel-vectors).  The RoI's
+//                    level, image and its per-axis TAP tables are staged in shared memory: the g
+//                    samples of a bin give up to 2g (pixel, weight) taps per axis, equal pixels
+//                    merged, computed ONCE per RoI and reused by every channel (north_star).  The
+//                    operator is separable, so a bin is sum_{y taps} sum_{x taps} wy*wx*F[y][x]:
+//                    typically 3x3 loads instead of 4 samples x 4 taps.  A warp owns an output bin
+//                    row (its y taps and row pointers stay in registers) and walks the bins of the
+//                    row; lanes = channel vectors: each 128-bit load covers 4 fp32 / 8 half
+//                    channels of one tap, a warp reads 512 contiguous bytes.
 //  * fwd_generic_kernel  any strides / any C / adaptive sampling: one thread per output element.
 #include "raf_device.cuh"
 #include "raf_host.h"
 
 namespace raf {
 
-constexpr int kTable = 64;  // max samples per axis (out_size * sampling_ratio) of the fast path
-
-struct AxisEntry {
-  int lo, hi;     // element offsets of the two taps (already multiplied by the axis stride)
-  float wl, wh;   // weights of hi / lo; both 0 when the sample is outside the map (reading S6)
+// One merged bilinear tap of an output bin along one axis: element offset of the pixel (already
+// multiplied by the axis stride) and its weight (y taps carry 1/count).
+struct FwdTap {
+  int off;
+  float w;
 };
 
-template <typename T, int G>
-__global__ void __launch_bounds__(256)
+constexpr int kFwdWarps = 8;   // max warps per CTA (one output bin row each, strided)
+
+// Merged taps of bin `bin` of one axis into tab[0..2g) (shared memory); returns the count.
+// Equal pixels are merged (weights summed in sample order); invalid samples (reading S6) give no tap.
+__device__ __forceinline__ int fwd_bin_taps(float start, float bsz, int bin, int g, int n, int stride,
+                                            float scale_w, FwdTap* tab) {
+  int cnt = 0;
+  if (g <= 2) {   // usual case: merge in registers
+    int pix[4] = {-1, -1, -1, -1};
+    float w[4] = {0.f, 0.f, 0.f, 0.f};
+    auto add = [&](int p, float v) {
+      bool found = false;
+#pragma unroll
+      for (int q = 0; q < 4; ++q)
+        if (q < cnt && pix[q] == p) { w[q] += v; found = true; }
+      if (!found) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+          if (q == cnt) { pix[q] = p; w[q] = v; }
+        ++cnt;
+      }
+    };
+    for (int i = 0; i < g; ++i) {
+      const AxisTap t = axis_tap(sample_coord(start, bsz, bin, i, g), n);
+      if (!t.valid) continue;
+      add(t.lo, t.wh * scale_w);
+      add(t.hi, t.wl * scale_w);
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      if (q < 2 * g) { tab[q].off = (q < cnt ? pix[q] : 0) * stride; tab[q].w = w[q]; }
+    return cnt;
+  }
+  for (int i = 0; i < g; ++i) {
+    const AxisTap t = axis_tap(sample_coord(start, bsz, bin, i, g), n);
+    if (!t.valid) continue;
+    const int po[2] = {t.lo * stride, t.hi * stride};
+    const float pw[2] = {t.wh * scale_w, t.wl * scale_w};
+    for (int h = 0; h < 2; ++h) {
+      int q = 0;
+      while (q < cnt && tab[q].off != po[h]) ++q;
+      if (q < cnt) tab[q].w += pw[h];
+      else { tab[cnt].off = po[h]; tab[cnt].w = pw[h]; ++cnt; }
+    }
+  }
+  return cnt;
+}
+
+// acc += sum_{a < NY, b < NX} (yw[a] * xw[b]) * F[rp[a] + xo[b]]: all NY*NX loads are issued before
+// the first use (memory-level parallelism is what bounds this kernel).
+template <typename T, int NY, int NX>
+__device__ __forceinline__ void fwd_accumulate(const T* rp0, const T* rp1, const T* rp2, const T* rp3,
+                                               const float (&yw)[4], const int (&xo)[4],
+                                               const float (&xw)[4], float (&acc)[Vec16<T>::N]) {
+  constexpr int VN = Vec16<T>::N;
+  const T* rp[4] = {rp0, rp1, rp2, rp3};
+  float v[NY][NX][VN];
+#pragma unroll
+  for (int a = 0; a < NY; ++a)
+#pragma unroll
+    for (int b = 0; b < NX; ++b) Vec16<T>::load(rp[a] + xo[b], v[a][b]);
+#pragma unroll
+  for (int a = 0; a < NY; ++a)
+#pragma unroll
+    for (int b = 0; b < NX; ++b) {
+      const float w = yw[a] * xw[b];
+#pragma unroll
+      for (int j = 0; j < VN; ++j) acc[j] = fmaf(w, v[a][b][j], acc[j]);
+    }
+}
+
+template <typename T, int NY>
+__device__ __forceinline__ void fwd_dispatch_x(int nx, const T* rp0, const T* rp1, const T* rp2, const T* rp3,
+                                               const float (&yw)[4], const int (&xo)[4], const float (&xw)[4],
+                                               float (&acc)[Vec16<T>::N]) {
+  switch (nx) {
+    case 1: fwd_accumulate<T, NY, 1>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+    case 2: fwd_accumulate<T, NY, 2>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+    case 3: fwd_accumulate<T, NY, 3>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+    default: fwd_accumulate<T, NY, 4>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+  }
+}
+
+// Channels-last forward.  CTA = (RoI, chunk of 32 channel-vectors); warp = output bin row(s);
+// lanes = channel vectors (16 bytes each: a warp-wide load covers 512 contiguous bytes).
+template <typename T>
+__global__ void __launch_bounds__(32 * kFwdWarps, 3)
 fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
-              int64_t os_w) {
+              int64_t os_w, int chunks) {
   using V = Vec16<T>;
   constexpr int VN = V::N;
-  __shared__ AxisEntry s_y[kTable], s_x[kTable];
-  __shared__ float s_inv_count;
-  __shared__ int s_level, s_b;
+  extern __shared__ __align__(16) unsigned char fwd_smem[];
+  const int g = a.sampling_ratio, slots = 2 * g;
+  const int PH = a.PH, PW = a.PW, nb = PH + PW;
+  FwdTap* s_tab = reinterpret_cast<FwdTap*>(fwd_smem);          // [PH + PW][slots]; y bins first
+  int* s_cnt = reinterpret_cast<int*>(s_tab + nb * slots);     // [PH + PW]
+  __shared__ int s_b;
 
-  const int k = blockIdx.x;
-  const int tid = threadIdx.y * blockDim.x + threadIdx.x;
-  const int g = (G > 0) ? G : a.sampling_ratio;
-  const int ny = a.PH * g, nx = a.PW * g;
+  const int k = blockIdx.x / chunks, chunk = blockIdx.x - k * chunks;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   const float* r = a.rois + 5 * (int64_t)k;
   const float r0 = __ldg(r), x1 = __ldg(r + 1), y1 = __ldg(r + 2), x2 = __ldg(r + 3), y2 = __ldg(r + 4);
   const int level = level_of(x1, y1, x2, y2, lv.L, a.finest_scale);
 
-  if (tid < ny + nx) {
-    const RoiGeom geo = roi_geom(x1, y1, x2, y2, lv.scale[level], a.PH, a.PW, g, a.aligned);
-    const bool isy = tid < ny;
-    const int s = isy ? tid : tid - ny;
-    const int p = s / g, i = s - p * g;
-    const float v = isy ? sample_coord(geo.sy, geo.bh, p, i, g) : sample_coord(geo.sx, geo.bw, p, i, g);
-    const AxisTap t = axis_tap(v, isy ? lv.h[level] : lv.w[level]);
-    const int stride = (int)(isy ? lv.sh[level] : lv.sw[level]);
-    AxisEntry e;
-    e.lo = t.lo * stride;
-    e.hi = t.hi * stride;
-    e.wl = t.valid ? t.wl : 0.0f;
-    e.wh = t.valid ? t.wh : 0.0f;
-    if (isy) s_y[s] = e; else s_x[s] = e;
-    if (tid == 0) {
-      s_inv_count = geo.inv_count;
-      s_level = level;
-      s_b = batch_index_of(r0, lv.n);
-    }
+  if ((int)threadIdx.x < nb) {
+    const int t = threadIdx.x;
+    const RoiGeom geo = roi_geom(x1, y1, x2, y2, lv.scale[level], PH, PW, g, a.aligned);
+    const bool isy = t < PH;
+    s_cnt[t] = isy ? fwd_bin_taps(geo.sy, geo.bh, t, g, lv.h[level], (int)lv.sh[level], geo.inv_count, s_tab + t * slots)
+                   : fwd_bin_taps(geo.sx, geo.bw, t - PH, g, lv.w[level], (int)lv.sw[level], 1.0f, s_tab + t * slots);
+    if (t == 0) s_b = batch_index_of(r0, lv.n);
   }
   __syncthreads();
 
   const int b = s_b;
-  const float inv_count = s_inv_count;
-  const int CV = lv.c / VN;
-  const int nbins = a.PH * a.PW;
-  T* out_k = out + (int64_t)k * os_k;
-  const T* base = (b >= 0) ? reinterpret_cast<const T*>(lv.data[level]) + (int64_t)b * lv.sn[level] : nullptr;
+  const int cv = chunk * 32 + lane;
+  if (cv * VN >= lv.c) return;
+  T* out_k = out + (int64_t)k * os_k + cv * VN;
+  const T* base = reinterpret_cast<const T*>(lv.data[level]) + (int64_t)(b >= 0 ? b : 0) * lv.sn[level] + cv * VN;
 
-  for (int bin = threadIdx.y; bin < nbins; bin += blockDim.y) {
-    const int ph = bin / a.PW, pw = bin - ph * a.PW;
-    for (int cv = threadIdx.x; cv < CV; cv += blockDim.x) {
+  for (int ph = warp; ph < PH; ph += nwarps) {
+    const int ny = (b >= 0) ? s_cnt[ph] : 0;
+    const FwdTap* ty = s_tab + ph * slots;
+    float yw[4];
+    int yo[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const FwdTap e = (q < slots) ? ty[q] : FwdTap{0, 0.f};
+      yo[q] = e.off;
+      yw[q] = e.w;
+    }
+    const T* rp0 = base + yo[0];
+    const T* rp1 = base + yo[1];
+    const T* rp2 = base + yo[2];
+    const T* rp3 = base + yo[3];
+    for (int pw = 0; pw < PW; ++pw) {
+      const int nx = s_cnt[PH + pw];
+      const FwdTap* tx = s_tab + (PH + pw) * slots;
       float acc[VN];
 #pragma unroll
       for (int j = 0; j < VN; ++j) acc[j] = 0.0f;
-      if (b >= 0) {
-        const T* bc = base + cv * VN;
-#pragma unroll(G > 0 ? G : 1)
-        for (int iy = 0; iy < g; ++iy) {
-          const AxisEntry ey = s_y[ph * g + iy];
-#pragma unroll(G > 0 ? G : 1)
-          for (int ix = 0; ix < g; ++ix) {
-            const AxisEntry ex = s_x[pw * g + ix];
-            const float w1 = __fmul_rn(ey.wh, ex.wh), w2 = __fmul_rn(ey.wh, ex.wl);
-            const float w3 = __fmul_rn(ey.wl, ex.wh), w4 = __fmul_rn(ey.wl, ex.wl);
-            float v1[VN], v2[VN], v3[VN], v4[VN];
-            V::load(bc + ey.lo + ex.lo, v1);
-            V::load(bc + ey.lo + ex.hi, v2);
-            V::load(bc + ey.hi + ex.lo, v3);
-            V::load(bc + ey.hi + ex.hi, v4);
+      if (ny > 0 && nx > 0) {
+        if (ny <= 4 && nx <= 4) {
+          int xo[4];
+          float xw[4];
 #pragma unroll
-            for (int j = 0; j < VN; ++j)
-              acc[j] += w1 * v1[j] + w2 * v2[j] + w3 * v3[j] + w4 * v4[j];
+          for (int q = 0; q < 4; ++q) {
+            const FwdTap e = (q < slots) ? tx[q] : FwdTap{0, 0.f};
+            xo[q] = e.off;
+            xw[q] = e.w;
+          }
+          switch (ny) {
+            case 1: fwd_dispatch_x<T, 1>(nx, rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+            case 2: fwd_dispatch_x<T, 2>(nx, rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+            case 3: fwd_dispatch_x<T, 3>(nx, rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+            default: fwd_dispatch_x<T, 4>(nx, rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+          }
+        } else {   // sampling_ratio > 2: walk the tap lists
+          for (int qa = 0; qa < ny; ++qa) {
+            const FwdTap ey = ty[qa];
+            for (int qb = 0; qb < nx; ++qb) {
+              const FwdTap ex = tx[qb];
+              float v[VN];
+              V::load(base + ey.off + ex.off, v);
+              const float w = ey.w * ex.w;
+#pragma unroll
+              for (int j = 0; j < VN; ++j) acc[j] = fmaf(w, v[j], acc[j]);
+            }
           }
         }
       }
-#pragma unroll
-      for (int j = 0; j < VN; ++j) acc[j] *= inv_count;
-      V::store(out_k + ph * os_h + pw * os_w + cv * VN, acc);
+      V::store(out_k + ph * os_h + pw * os_w, acc);
     }
   }
 }
@@ -145,16 +244,14 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
                          bool channels_last, cudaStream_t stream) {
   T* o = reinterpret_cast<T*>(out);
   const int g = a.sampling_ratio;
-  if (channels_last && g > 0 && a.PH * g <= kTable && a.PW * g <= kTable) {
+  if (channels_last && g > 0) {
     const int CV = lv.c / Vec16<T>::N;
-    int bx = 1;
-    while (bx < CV && bx < 256) bx <<= 1;
-    const dim3 block(bx, 256 / bx);
-    const dim3 grid(a.K);
-    if (g == 2)
-      fwd_cl_kernel<T, 2><<<grid, block, 0, stream>>>(lv, a, o, os[0], os[2], os[3]);
-    else
-      fwd_cl_kernel<T, 0><<<grid, block, 0, stream>>>(lv, a, o, os[0], os[2], os[3]);
+    const int chunks = (CV + 31) / 32;
+    const size_t smem = (size_t)(a.PH + a.PW) * (2 * g * sizeof(FwdTap) + sizeof(int));
+    int nw = a.PH < kFwdWarps ? a.PH : kFwdWarps;          // one warp per output bin row
+    while (32 * nw < a.PH + a.PW) ++nw;                     // the table set-up needs PH + PW threads
+    fwd_cl_kernel<T><<<(unsigned)((int64_t)a.K * chunks), 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2], os[3],
+                                                                                          chunks);
   } else {
     const int64_t total = (int64_t)a.K * lv.c * a.PH * a.PW;
     const int64_t blocks = (total + 255) / 256;

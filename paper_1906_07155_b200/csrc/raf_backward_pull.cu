@@ -113,7 +113,8 @@ __device__ __forceinline__ void pull_taps_item(const LevelsParam& lv, const RoiA
   for (int q = cnt; q < slots; ++q) { out[q].pb = tag | kPixMask; out[q].w = 0.0f; }
 }
 
-constexpr int kPrepThreads = 1024;
+constexpr int kPrepThreads = 256;
+constexpr int kPrepWarps = kPrepThreads / 32;
 
 // ---------------------------------------------------------------------------------------------
 // Stable bucketing by (level, image): key = level * N + batch_idx.  Feeds the pull backward
@@ -123,7 +124,7 @@ constexpr int kPrepThreads = 1024;
 //   boff[NK + 1]  start of every key's group (NK = L * N)
 //   bwin[K]       (optional) in bperm order: conservative window {ymin, ymax, xmin, xmax} of the
 //                 pixels the RoI's samples can touch on its level (empty: ymin > ymax)
-// Block 0 of pull_prep_kernel (the other blocks write the tap tables, same launch): 32 warps; warp w owns the contiguous RoI range [w*q, (w+1)*q).  cnt[w][key] first
+// Block 0 of pull_prep_kernel (the other blocks write the tap tables, same launch): 8 warps; warp w owns the contiguous RoI range [w*q, (w+1)*q).  cnt[w][key] first
 // counts, then (after a scan over keys, warps minor) holds the next free slot of (key, warp):
 // warp-private rows, so neither atomics nor block barriers inside the walks.
 // ---------------------------------------------------------------------------------------------
@@ -144,7 +145,7 @@ __device__ __forceinline__ void axis_window(float start, float bin, int P, int g
 __global__ void __launch_bounds__(kPrepThreads, 1)
 pull_prep_kernel(const LevelsParam lv, const RoiArgs a, int32_t* __restrict__ bperm,
                  int32_t* __restrict__ boff, int4* __restrict__ bwin, PullTap* __restrict__ taps) {
-  extern __shared__ int s_cnt[];  // [32][NK + 1] then [NK + 1] totals/offsets
+  extern __shared__ int s_cnt[];  // [kPrepWarps][NK + 1] then [NK + 1] totals/offsets
   if (blockIdx.x > 0) {           // blocks 1.. : tap tables (independent of the bucketing)
     const int64_t idx = (int64_t)(blockIdx.x - 1) * kPrepThreads + threadIdx.x;
     if (idx < (int64_t)a.K * (a.PH + a.PW)) pull_taps_item(lv, a, idx, taps);
@@ -152,11 +153,11 @@ pull_prep_kernel(const LevelsParam lv, const RoiArgs a, int32_t* __restrict__ bp
   }
   const int K = a.K, L = lv.L, N = lv.n;
   const int NK = L * N, NK1 = NK + 1;
-  int* s_tot = s_cnt + 32 * NK1;
+  int* s_tot = s_cnt + kPrepWarps * NK1;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int q = ((K + 31) / 32 + 31) & ~31;  // per-warp range, multiple of 32
+  const int q = ((K + kPrepWarps - 1) / kPrepWarps + 31) & ~31;  // per-warp range, multiple of 32
   const int lo = warp * q, hi = min(K, lo + q);
-  for (int i = tid; i < 32 * NK1 + NK1; i += kPrepThreads) s_cnt[i] = 0;
+  for (int i = tid; i < kPrepWarps * NK1 + NK1; i += kPrepThreads) s_cnt[i] = 0;
   __syncthreads();
 
   auto key_of = [&](int k) -> int {
@@ -179,7 +180,7 @@ pull_prep_kernel(const LevelsParam lv, const RoiArgs a, int32_t* __restrict__ bp
   // totals per key
   for (int key = tid; key < NK1; key += kPrepThreads) {
     int t = 0;
-    for (int w = 0; w < 32; ++w) t += s_cnt[w * NK1 + key];
+    for (int w = 0; w < kPrepWarps; ++w) t += s_cnt[w * NK1 + key];
     s_tot[key] = t;
   }
   __syncthreads();
@@ -201,7 +202,7 @@ pull_prep_kernel(const LevelsParam lv, const RoiArgs a, int32_t* __restrict__ bp
   for (int key = tid; key < NK1; key += kPrepThreads) {
     if (key <= NK) boff[key] = s_tot[key];  // boff[NK] = number of kept RoIs
     int run = s_tot[key];
-    for (int w = 0; w < 32; ++w) {
+    for (int w = 0; w < kPrepWarps; ++w) {
       const int c = s_cnt[w * NK1 + key];
       s_cnt[w * NK1 + key] = run;
       run += c;
@@ -234,7 +235,7 @@ pull_prep_kernel(const LevelsParam lv, const RoiArgs a, int32_t* __restrict__ bp
   }
 }
 
-size_t bucket_smem_bytes(int L, int N) { return (size_t)33 * ((size_t)L * N + 1) * sizeof(int); }
+size_t bucket_smem_bytes(int L, int N) { return (size_t)(kPrepWarps + 1) * ((size_t)L * N + 1) * sizeof(int); }
 
 int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, int32_t* boff, int4* bwin,
                      PullTap* taps, cudaStream_t stream) {
@@ -285,7 +286,13 @@ __device__ __forceinline__ void fma4(float4& acc, float w, const float4& v) {
   acc.z = fmaf(w, v.z, acc.z); acc.w = fmaf(w, v.w, acc.w);
 }
 
-constexpr int kNC = 64;            // candidates per build/consume pass
+#ifndef RAF_PULL_NC
+#define RAF_PULL_NC 16
+#endif
+#ifndef RAF_PULL_MINB
+#define RAF_PULL_MINB 4
+#endif
+constexpr int kNC = RAF_PULL_NC;   // candidates per build/consume pass
 constexpr int kMaxTapChunks = 4;   // <= 128 taps per axis (eligibility checked on the host)
 constexpr uint32_t kOffMask = 0x00ffffffu;
 
@@ -299,17 +306,25 @@ struct __align__(16) PullInfo {
   float w1;
 };
 
+// One contribution to a pixel: element offset into grad_out (k*gs_k + ph*gs_h + pw*gs_w) and the
+// weight wy * wx.  Up to four per (candidate, pixel) in the fast path.
+struct PullPair {
+  int off;
+  float w;
+};
+
 template <typename T, bool kFull>
-__global__ void __launch_bounds__(kPullThreads, 4)
+__global__ void __launch_bounds__(kPullThreads, RAF_PULL_MINB)
 bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gout, int gs_k,
                 int gs_h, int gs_w, const int32_t* __restrict__ bperm,
                 const int32_t* __restrict__ boff, const int4* __restrict__ bwin,
                 const PullTap* __restrict__ taps, const PullTiles tiles, int accumulate) {
-  __shared__ int s_k[kPullThreads];
-  __shared__ int s_wcount[kPullThreads / 32];
+  __shared__ int s_k[2 * kPullThreads];
+  __shared__ int s_wcount[2 * kPullThreads / 32];
   __shared__ int s_goff[kNC];                          // k * gs_k
   __shared__ PullInfo s_info[kNC][16];                 // [c][0..7] rows, [c][8..15] columns
-  __shared__ unsigned char s_cnt[16][kNC];             // entry counts, transposed (ballot-friendly)
+  __shared__ __align__(16) PullPair s_pair[64][4 * kNC + 2];   // contributions per (pixel, candidate); padded rows
+  __shared__ unsigned char s_pc[64][kNC];              // their number; 255: walk the masks instead
   extern __shared__ uint32_t s_mask[];                 // [kNC][16][nq]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -344,24 +359,29 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
   const int bbeg = boff[key], bend = boff[key + 1];
   int npass = 0;
 
-  for (int s0 = bbeg; s0 < bend; s0 += kPullThreads) {
-    // ---- (A) candidates of this scan chunk, order preserved ------------------------------------
-    bool hit = false;
-    if (s0 + tid < bend) {
-      const int4 win = __ldg(bwin + s0 + tid);   // {ymin, ymax, xmin, xmax}, conservative; empty: ymin > ymax
-      hit = (win.x <= y1) && (win.y >= y0) && (win.z <= x1) && (win.w >= x0);
-    }
-    const unsigned m = __ballot_sync(0xffffffffu, hit);
-    if (lane == 0) s_wcount[warp] = __popc(m);
+  for (int s0 = bbeg; s0 < bend; s0 += 2 * kPullThreads) {
+    // ---- (A) candidates of this scan chunk (512 bucket entries, two per thread, all loads issued
+    //      together), order preserved ------------------------------------------------------------
+    const int ia = s0 + tid, ib = s0 + kPullThreads + tid;
+    int4 wa = make_int4(0x7fffffff, -1, 0x7fffffff, -1), wb = wa;
+    int ka = 0, kb = 0;
+    if (ia < bend) { wa = __ldg(bwin + ia); ka = __ldg(bperm + ia); }   // {ymin, ymax, xmin, xmax}, conservative
+    if (ib < bend) { wb = __ldg(bwin + ib); kb = __ldg(bperm + ib); }
+    const bool hita = (wa.x <= y1) && (wa.y >= y0) && (wa.z <= x1) && (wa.w >= x0);
+    const bool hitb = (wb.x <= y1) && (wb.y >= y0) && (wb.z <= x1) && (wb.w >= x0);
+    const unsigned ma = __ballot_sync(0xffffffffu, hita), mb = __ballot_sync(0xffffffffu, hitb);
+    if (lane == 0) { s_wcount[warp] = __popc(ma); s_wcount[kPullThreads / 32 + warp] = __popc(mb); }
     __syncthreads();
-    int before = 0, ncand = 0;
+    int befa = 0, befb = 0, ncand = 0;
 #pragma unroll
-    for (int w = 0; w < kPullThreads / 32; ++w) {
+    for (int w = 0; w < 2 * kPullThreads / 32; ++w) {
       const int cnt = s_wcount[w];
-      if (w < warp) before += cnt;
+      if (w < warp) befa += cnt;
+      if (w < kPullThreads / 32 + warp) befb += cnt;
       ncand += cnt;
     }
-    if (hit) s_k[before + __popc(m & ((1u << lane) - 1u))] = __ldg(bperm + s0 + tid);
+    if (hita) s_k[befa + __popc(ma & ((1u << lane) - 1u))] = ka;
+    if (hitb) s_k[befb + __popc(mb & ((1u << lane) - 1u))] = kb;
     __syncthreads();
 
     for (int p0 = 0; p0 < ncand; p0 += kNC) {
@@ -407,9 +427,30 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
             inf.w1 = e.w;
           }
           s_info[c][lane] = inf;
-          s_cnt[lane][c] = (unsigned char)min(cnt, 255);
         }
         if (lane == 0) s_goff[c] = k * gs_k;
+        __syncwarp();
+        // lanes = pixels now: expand (row entries) x (column entries) into the pixel's pair slots
+        const int goff = k * gs_k;
+        for (int p = lane; p < 8 * npy; p += 32) {
+          const PullInfo iy = s_info[c][p >> 3], ix = s_info[c][8 + (p & 7)];
+          const uint32_t cy = iy.m0 >> 24, cx = ix.m0 >> 24;
+          const int oy0 = goff + (int)(iy.m0 & kOffMask), oy1 = goff + (int)iy.off1;
+          const int ox0 = (int)(ix.m0 & kOffMask), ox1 = (int)ix.off1;
+          uint4 e01, e23;   // order: (y0,x0) (y0,x1) (y1,x0) (y1,x1), absent ones skipped
+          e01.x = (uint32_t)(oy0 + ox0); e01.y = __float_as_uint(iy.w0 * ix.w0);
+          if (cx >= 2) {
+            e01.z = (uint32_t)(oy0 + ox1); e01.w = __float_as_uint(iy.w0 * ix.w1);
+            e23.x = (uint32_t)(oy1 + ox0); e23.y = __float_as_uint(iy.w1 * ix.w0);
+          } else {
+            e01.z = (uint32_t)(oy1 + ox0); e01.w = __float_as_uint(iy.w1 * ix.w0);
+            e23.x = 0u; e23.y = 0u;
+          }
+          e23.z = (uint32_t)(oy1 + ox1); e23.w = __float_as_uint(iy.w1 * ix.w1);
+          *reinterpret_cast<uint4*>(&s_pair[p][4 * c]) = e01;
+          *reinterpret_cast<uint4*>(&s_pair[p][4 * c + 2]) = e23;
+          s_pc[p][c] = (cy == 0 || cx == 0) ? 0 : ((cy > 2 || cx > 2) ? 255 : (unsigned char)(cy * cx));
+        }
       }
       __syncthreads();
 
@@ -419,81 +460,76 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
       for (int i = 0; i < npy; ++i) {
         const int j = (warp + i) & 7;
         if (j >= npx) continue;
-        {
-          float* gp = gtile + i * sh + j * sw;
-          float4 accA = make_float4(0.f, 0.f, 0.f, 0.f), accB = accA;
-          if (accumulate || npass) {
-            if (actA) accA = *reinterpret_cast<const float4*>(gp);
-            if (actB) accB = *reinterpret_cast<const float4*>(gp + 128);
-          }
-          unsigned cm[2];
-          cm[0] = __ballot_sync(0xffffffffu, lane < nc && s_cnt[i][lane] != 0 && s_cnt[8 + j][lane] != 0);
-          cm[1] = __ballot_sync(0xffffffffu, 32 + lane < nc && s_cnt[i][32 + lane] != 0 && s_cnt[8 + j][32 + lane] != 0);
-#pragma unroll
-          for (int half = 0; half < 2; ++half) {
-            unsigned mm = cm[half];
-            while (mm) {
-              const int c = half * 32 + __ffs(mm) - 1;
-              mm &= mm - 1;
-              const PullInfo iy = s_info[c][i];
-              const PullInfo ix = s_info[c][8 + j];
-              const T* gk = goutA + s_goff[c];
-              const uint32_t cy = iy.m0 >> 24, cx = ix.m0 >> 24;
-              if (cy <= 2 && cx <= 2) {
-                const uint32_t oy0 = iy.m0 & kOffMask, ox0 = ix.m0 & kOffMask;
-                {
-                  const T* p = gk + (oy0 + ox0);
-                  const float w = iy.w0 * ix.w0;
-                  fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
-                }
-                if (cx == 2) {
-                  const T* p = gk + (oy0 + ix.off1);
-                  const float w = iy.w0 * ix.w1;
-                  fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
-                }
-                if (cy == 2) {
-                  {
-                    const T* p = gk + (iy.off1 + ox0);
-                    const float w = iy.w1 * ix.w0;
-                    fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
-                  }
-                  if (cx == 2) {
-                    const T* p = gk + (iy.off1 + ix.off1);
-                    const float w = iy.w1 * ix.w1;
-                    fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
-                  }
-                }
-              } else {   // rare: more than two entries on an axis -> walk the ballot masks
-                const int k = s_k[p0 + c];
-                const PullTap* ty = taps + (int64_t)k * (nty + ntx);
-                const PullTap* tx = ty + nty;
-                for (int qy = 0; qy < nq; ++qy) {
-                  unsigned my = s_mask[(c * 16 + i) * nq + qy];
-                  while (my) {
-                    const PullTap ey = ty[qy * 32 + __ffs(my) - 1];
-                    my &= my - 1;
-                    const T* gy = gk + (ey.pb >> 24) * (uint32_t)gs_h;
-                    for (int qx = 0; qx < nq; ++qx) {
-                      unsigned mx = s_mask[(c * 16 + 8 + j) * nq + qx];
-                      while (mx) {
-                        const PullTap ex = tx[qx * 32 + __ffs(mx) - 1];
-                        mx &= mx - 1;
-                        const T* p = gy + (ex.pb >> 24) * (uint32_t)gs_w;
-                        const float w = ey.w * ex.w;
-                        fma4(accA, w, ldg4<T>(p)); fma4(accB, w, ldg4<T>(p + dAB));
-                      }
-                    }
+        const int p = i * 8 + j;
+        float* gp = gtile + i * sh + j * sw;
+        float4 accA = make_float4(0.f, 0.f, 0.f, 0.f), accB = accA;
+        if (accumulate || npass) {
+          if (actA) accA = *reinterpret_cast<const float4*>(gp);
+          if (actB) accB = *reinterpret_cast<const float4*>(gp + 128);
+        }
+        // pair count of every candidate on this pixel: lane c holds candidate c's
+        const unsigned pcv = (lane < nc) ? s_pc[p][lane] : 0u;
+        unsigned mm = __ballot_sync(0xffffffffu, pcv != 0);
+        while (mm) {
+          const int c = __ffs(mm) - 1;
+          mm &= mm - 1;
+          const unsigned np = __shfl_sync(0xffffffffu, pcv, c);
+          if (np != 255u) {
+            const PullPair* sp = &s_pair[p][4 * c];
+            const uint4 e01 = *reinterpret_cast<const uint4*>(sp);
+            {
+              const T* q = goutA + (int)e01.x;
+              const float w = __uint_as_float(e01.y);
+              fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+            }
+            if (np > 1) {
+              const T* q = goutA + (int)e01.z;
+              const float w = __uint_as_float(e01.w);
+              fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+            }
+            if (np > 2) {
+              const uint4 e23 = *reinterpret_cast<const uint4*>(sp + 2);
+              {
+                const T* q = goutA + (int)e23.x;
+                const float w = __uint_as_float(e23.y);
+                fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+              }
+              if (np > 3) {
+                const T* q = goutA + (int)e23.z;
+                const float w = __uint_as_float(e23.w);
+                fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+              }
+            }
+          } else {   // rare: more than two entries on an axis -> walk the ballot masks
+            const int k = s_k[p0 + c];
+            const T* gk = goutA + s_goff[c];
+            const PullTap* ty = taps + (int64_t)k * (nty + ntx);
+            const PullTap* tx = ty + nty;
+            for (int qy = 0; qy < nq; ++qy) {
+              unsigned my = s_mask[(c * 16 + i) * nq + qy];
+              while (my) {
+                const PullTap ey = ty[qy * 32 + __ffs(my) - 1];
+                my &= my - 1;
+                const T* gy = gk + (ey.pb >> 24) * (uint32_t)gs_h;
+                for (int qx = 0; qx < nq; ++qx) {
+                  unsigned mx = s_mask[(c * 16 + 8 + j) * nq + qx];
+                  while (mx) {
+                    const PullTap ex = tx[qx * 32 + __ffs(mx) - 1];
+                    mx &= mx - 1;
+                    const T* q = gy + (ex.pb >> 24) * (uint32_t)gs_w;
+                    const float w = ey.w * ex.w;
+                    fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
                   }
                 }
               }
             }
           }
-          if (actA) *reinterpret_cast<float4*>(gp) = accA;
-          if (actB) *reinterpret_cast<float4*>(gp + 128) = accB;
         }
+        if (actA) *reinterpret_cast<float4*>(gp) = accA;
+        if (actB) *reinterpret_cast<float4*>(gp + 128) = accB;
       }
       ++npass;
-      if (p0 + kNC < ncand || s0 + kPullThreads < bend)
+      if (p0 + kNC < ncand || s0 + 2 * kPullThreads < bend)
         __syncthreads();  // tables and s_k are rewritten by the next pass / scan chunk
     }
   }

@@ -180,7 +180,7 @@ def test_backward_config1(layout, flags):
 @pytest.mark.parametrize("layout,flags", VARIANTS)
 @pytest.mark.parametrize("index,dtype,kw", [
     (2, "f32", dict(n_img=2, per_img=96, channels=64)),
-    (2, "f32", dict(n_img=1, per_img=300, channels=256)),   # > 256 RoIs in one bucket: two scan chunks
+    (2, "f32", dict(n_img=1, per_img=300, channels=256)),   # one big (level, image) bucket, full 256-channel chunk
     (4, "bf16", dict(n_img=2, per_img=40, channels=32)),
     (5, "bf16", dict(n_img=3, per_img=64, channels=32)),
     (5, "f16", dict(n_img=2, per_img=50, channels=36)),
@@ -197,6 +197,50 @@ def test_backward_reduced_configs(index, dtype, kw, layout, flags):
 def test_backward_variants(P, g, aligned, layout, flags):
     wl = inputs.make_workload(5, n_img=2, per_img=24, channels=8)
     _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned, flags=flags)
+
+
+def _single_level_case(K, C, H, W, side_lo, side_hi, seed, flags, P=(7, 7), g=2, dtype="f32"):
+    """Many RoIs on ONE small map: exercises the pull kernel's multi-pass tiles (more than 16
+    candidates per tile), scan chunks (more than 512 RoIs per bucket) and, with tiny boxes, the
+    slow path (more than two tap entries per pixel row / column)."""
+    rng = np.random.default_rng(seed)
+    side = rng.uniform(side_lo, side_hi, (K, 2))
+    cx, cy = rng.uniform(-1, W + 1, K), rng.uniform(-1, H + 1, K)
+    rois = np.stack([np.zeros(K), cx - side[:, 0] / 2, cy - side[:, 1] / 2, cx + side[:, 0] / 2,
+                     cy + side[:, 1] / 2], 1).astype(np.float32)
+    gout = rng.standard_normal((K, C, *P)).astype(np.float32)
+    shapes, scales = [(1, C, H, W)], [1.0]
+    got, go_exact = T.gpu_backward(shapes, scales, gout, rois, g, True, 56.0, "cl", dtype, flags)
+    ref, S = R.backward(shapes, scales, go_exact, rois, P, g, True, 56.0)
+    return T.assert_backward_close(got, ref, S)
+
+
+@pytest.mark.parametrize("flags", [0, B.RAF_DETERMINISTIC, B.RAF_ATOMIC])
+def test_backward_dense_tiles_and_big_buckets(flags):
+    _single_level_case(K=700, C=16, H=24, W=40, side_lo=4, side_hi=20, seed=11, flags=flags)
+
+
+@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC])
+@pytest.mark.parametrize("C,dtype", [(8, "f32"), (320, "f32"), (264, "bf16")])
+def test_backward_tiny_boxes_many_entries_per_pixel(flags, C, dtype):
+    # boxes of 0.3 .. 3 px: bins narrower than half a pixel -> up to 7 entries per row / column
+    _single_level_case(K=90, C=C, H=17, W=19, side_lo=0.3, side_hi=3.0, seed=12, flags=flags, dtype=dtype)
+
+
+@pytest.mark.parametrize("P,g", [((14, 14), 2), ((9, 20), 3)])
+def test_backward_many_taps_dense(P, g):
+    # more than 32 taps per axis (two / four ballot chunks) on a dense map
+    _single_level_case(K=120, C=12, H=20, W=20, side_lo=2, side_hi=18, seed=13, flags=0, P=P, g=g)
+
+
+def test_backward_pull_unsupported_sizes_fall_back():
+    # 32 bins x 2*4 slots = 256 taps per axis: beyond the pull kernel's tables -> atomic path in
+    # auto mode, refusal when determinism is demanded
+    _single_level_case(K=20, C=8, H=20, W=20, side_lo=2, side_hi=18, seed=14, flags=0, P=(32, 32), g=4)
+    with pytest.raises(B.RafError) as e:
+        _single_level_case(K=20, C=8, H=20, W=20, side_lo=2, side_hi=18, seed=14, flags=B.RAF_DETERMINISTIC,
+                           P=(32, 32), g=4)
+    assert e.value.status == -5
 
 
 def test_backward_degenerate_and_invalid_rois():

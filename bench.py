@@ -32,8 +32,8 @@ UNIT = "RoIs/s"
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based)")
     ap.add_argument("--layout", default="cl", choices=["cl", "nchw"])
@@ -308,10 +308,8 @@ def run_ours(args):
     fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, g, aligned, fs)
     ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz)
     peak, peak_src = peaks()
-    traffic = {}
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(f"config{args.config}", {})
+    from paper_1906_07155_b200 import ncu_traffic
+    traffic = ncu_traffic.TRAFFIC_BYTES.get(args.config, {}) if args.layout == "cl" and args.backward == "auto" else {}
     legs = {"fwd": (ab["fwd"], fwd_ms)}
     if bwd_ms is not None:
         legs["bwd"] = (ab["bwd"], bwd_ms)
@@ -321,7 +319,9 @@ def run_ours(args):
         by, ms = legs[name]
         ach = by / (ms * 1e-3) / 1e9
         return {"bound": "hbm", "kernel": name, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": traffic.get(name), "algorithmic_bytes": by, "ms": ms, "peak_source": peak_src}
+                "traffic": traffic.get(name), "traffic_source": traffic.get("source"), "algorithmic_bytes": by, "ms": ms,
+                "peak_source": peak_src,
+                "note": "ms = CUDA-event time of the whole C-ABI call of this leg (bwd: prep launch + pull kernel)"}
 
     step_ms = total_ms / args.steps
     step_bytes = ab["fwd"] + (ab["bwd"] if cfg.backward else 0)

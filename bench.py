@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--graph", action="store_true", help="replay each step from a CUDA graph")
+    ap.add_argument("--no-reuse-prep", action="store_true",
+                    help="backward rebuilds its RoI buckets / tap tables instead of reusing the forward's (RAF_REUSE_PREP)")
     return ap.parse_args()
 
 
@@ -210,6 +212,9 @@ def run_ours(args):
     PH, PW = cfg.out_size
     g, aligned, fs = cfg.sampling_ratio, cfg.aligned, cfg.finest_scale
     flags = {"auto": 0, "atomic": B.RAF_ATOMIC, "deterministic": B.RAF_DETERMINISTIC}[args.backward]
+    if not args.no_reuse_prep and args.backward != "atomic":
+        flags |= B.RAF_REUSE_PREP   # a step runs the forward first, on the same RoIs and workspace: its launch
+                                    # already wrote the backward's RoI buckets / tap tables (include/raf.h)
 
     def lay(t):   # logical NCHW tensor -> requested physical layout
         return t.contiguous() if args.layout == "nchw" else t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
@@ -289,7 +294,7 @@ def run_ours(args):
         dist.barrier()
     launches = B.launch_count() - launches0
     if graphs:   # replayed launches are not seen by the library's counter: count per captured step
-        launches = args.steps * (1 + ((1 + L) if args.backward == "atomic" else 2) * cfg.backward)
+        launches = args.steps * (1 + ((1 + L) if args.backward == "atomic" else (1 if flags & B.RAF_REUSE_PREP else 2)) * cfg.backward)
     total_ms = ev[0][0].elapsed_time(ev[-1][2])
     if world > 1:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
@@ -332,6 +337,7 @@ def run_ours(args):
                        "out_size": [PH, PW], "levels": L, "layout": args.layout, "parallelism": f"replicas x{world} (shard by image, no collective)",
                        "l2_protocol": f"inputs rotate over {R} independent copies ({R * ws_set / 1e6:.0f} MB >> L2 {l2 / 1e6:.0f} MB)",
                        "backward": args.backward if cfg.backward else "none",
+                       "reuse_prep": bool(flags & B.RAF_REUSE_PREP) if cfg.backward else False,
                        "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
             "roofline": roof(dom),
             "roofline_all": {k: roof(k) for k in legs} | {"step": {"achieved": step_bytes / (step_ms * 1e-3) / 1e9,

@@ -59,7 +59,14 @@ enum {
   RAF_DETERMINISTIC = 2,  /* REQUIRE the bit-reproducible pull variant (K3d); RAF_ERR_UNSUPPORTED
                              if the layout is not eligible (needs channels-last, C % 4 == 0,
                              sampling_ratio > 0, L*N <= 1500)                                       */
-  RAF_ATOMIC = 4          /* force the atomic scatter variant (zero-fill + red.global.add.v4.f32)  */
+  RAF_ATOMIC = 4,         /* force the atomic scatter variant (zero-fill + red.global.add.v4.f32)  */
+  RAF_REUSE_PREP = 8      /* the workspace still holds what roi_align_fpn_forward wrote into it when
+                             called with the SAME rois (contents and K), level shapes and scales,
+                             out_h/out_w, sampling_ratio, aligned, finest_scale and workspace pointer:
+                             the backward then skips its own RoI bucketing / tap-table launch.  The
+                             forward always leaves the workspace in that state when it returns RAF_OK;
+                             with different arguments the result is undefined (but memory-safe only
+                             if K and the level shapes match).                                       */
 };
 /* With neither RAF_DETERMINISTIC nor RAF_ATOMIC the library picks the pull variant when eligible
  * and the atomic variant otherwise. */
@@ -84,7 +91,9 @@ int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, i
  *   out          DEVICE, dtype = `dtype`, logical [K,C,out_h,out_w] addressed through
  *                out_strides (HOST array of 4 element strides); row k = RoI k (original order)
  *   sampling_ratio  > 0: fixed grid; 0: adaptive gh = ceil(roi_h/out_h), gw = ceil(roi_w/out_w)
- *   aligned      != 0: half-pixel shift, no minimum box size; 0: legacy (no shift, size >= 1)   */
+ *   aligned      != 0: half-pixel shift, no minimum box size; 0: legacy (no shift, size >= 1)
+ *   ws           written: RoI buckets and tap tables that a following roi_align_fpn_backward on the
+ *                same arguments may reuse (RAF_REUSE_PREP)                                          */
 int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
                           int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
                           void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,
@@ -95,7 +104,7 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
  *                shapes as the features.  Overwritten (every element written: zero or sum) unless
  *                RAF_ACCUMULATE.
  *   grad_out     DEVICE, dtype = gout_dtype, logical [K,C,out_h,out_w] through gout_strides (HOST)
- *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC                                              */
+ *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP                   */
 int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
                            const void* grad_out, const int64_t* gout_strides, const float* rois,
                            int K, int out_h, int out_w, int sampling_ratio, int aligned,

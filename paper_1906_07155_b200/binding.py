@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libraf.so")
 
 RAF_F32, RAF_F16, RAF_BF16 = 0, 1, 2
-RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC = 1, 2, 4
+RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC, RAF_REUSE_PREP = 1, 2, 4, 8
 _DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_BF16}
 
 EXPORTS = [

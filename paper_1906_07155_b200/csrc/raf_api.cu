@@ -6,6 +6,7 @@
 
 #include "raf_device.cuh"
 #include "raf_host.h"
+#include "raf_pull_prep.cuh"
 
 namespace raf {
 
@@ -103,6 +104,17 @@ static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
   return w;
 }
 
+// The pull backward's prep tables can be built for these arguments (layout-independent part of the
+// pull eligibility; the forward uses the same test before it writes them into the workspace).
+static bool prep_possible(const raf_level* lv, int L, int sampling_ratio) {
+  if (sampling_ratio <= 0 || (int64_t)L * lv[0].n + 1 > kBoffInts) return false;
+  if (bucket_smem_bytes(L, lv[0].n) > 200 * 1024) return false;
+  if ((size_t)(kMaxLevels + 1) * ((size_t)L * lv[0].n + 1) * sizeof(int) > 200 * 1024) return false;
+  for (int l = 0; l < L; ++l)   // tap tables keep pixel indices in 24 bits
+    if (lv[l].h >= 0xffffff || lv[l].w >= 0xffffff) return false;
+  return true;
+}
+
 size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,
                                      int flags) {
   (void)L; (void)flags;
@@ -144,7 +156,18 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
   const int vec = (int)(16 / esize(dtype));
   const bool cl = levels_vectorizable(feats, L, vec, esize(dtype)) &&
                   tensor_vectorizable(out, out_strides, vec, esize(dtype));
-  return launch_forward(p, dtype, a, out, out_strides, cl, (cudaStream_t)stream);
+  // the workspace receives the pull backward's prep tables (consumed by RAF_REUSE_PREP)
+  PullPrepOut po{nullptr, nullptr, nullptr, nullptr, 0};
+  const bool with_prep = prep_possible(feats, L, sampling_ratio);
+  if (with_prep) {
+    const WsLayout w = ws_layout(K, out_h, out_w, sampling_ratio);
+    char* base = reinterpret_cast<char*>(ws);
+    po.bperm = reinterpret_cast<int32_t*>(base + w.bperm);
+    po.boff = reinterpret_cast<int32_t*>(base + w.boff);
+    po.bwin = reinterpret_cast<int4*>(base + w.bwin);
+    po.taps = reinterpret_cast<PullTap*>(base + w.taps);
+  }
+  return launch_forward(p, dtype, a, out, out_strides, cl, with_prep ? &po : nullptr, (cudaStream_t)stream);
 }
 
 int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
@@ -157,7 +180,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (rc) return rc;
   if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
-  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP)) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
   if (!gout_strides) return RAF_ERR_NULL;
   for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
@@ -173,10 +196,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                   (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype)));
 
   // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
-  bool pull_ok = cl && sampling_ratio > 0 && (int64_t)L * grad_feats[0].n + 1 <= kBoffInts &&
-                 bucket_smem_bytes(L, grad_feats[0].n) <= 200 * 1024;
-  for (int l = 0; l < L; ++l)   // tap tables keep pixel indices in 24 bits
-    if (grad_feats[l].h >= 0xffffff || grad_feats[l].w >= 0xffffff) pull_ok = false;
+  const bool pull_ok = cl && prep_possible(grad_feats, L, sampling_ratio);
   if (pull_ok && !(flags & RAF_ATOMIC)) {
     const WsLayout w = ws_layout(K, out_h, out_w, sampling_ratio);
     char* base = reinterpret_cast<char*>(ws);
@@ -184,8 +204,10 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
     int32_t* boff = reinterpret_cast<int32_t*>(base + w.boff);
     int4* bwin = reinterpret_cast<int4*>(base + w.bwin);
     PullTap* taps = reinterpret_cast<PullTap*>(base + w.taps);
-    rc = launch_pull_prep(p, a, bperm, boff, bwin, taps, st);
-    if (rc) return rc;
+    if (!(flags & RAF_REUSE_PREP)) {   // else: written by roi_align_fpn_forward on the same arguments
+      rc = launch_pull_prep(p, a, bperm, boff, bwin, taps, st);
+      if (rc) return rc;
+    }
     rc = launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, bperm, boff, bwin, taps,
                               (flags & RAF_ACCUMULATE) ? 1 : 0, st);
     if (rc != RAF_ERR_UNSUPPORTED) return rc;

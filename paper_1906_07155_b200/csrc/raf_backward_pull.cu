@@ -30,13 +30,13 @@
 // Tiles of the coarsest level are scheduled first (most RoIs per pixel).
 #include "raf_device.cuh"
 #include "raf_host.h"
+#include "raf_pull_prep.cuh"
 
 namespace raf {
 
 constexpr int kPullThreads = 256;
 constexpr int kTW = 8;   // tile columns (register accumulators per thread)
 constexpr int kTH = 8;   // tile rows = warps per CTA
-constexpr uint32_t kPixMask = 0x00ffffffu;   // tap.pb = pixel | bin << 24; pixel == kPixMask: empty slot
 
 struct PullTiles {
   int32_t order[kMaxLevels];      // level processed at position i (coarsest first)
@@ -47,195 +47,13 @@ struct PullTiles {
   int32_t chunks;                 // channel chunks of 256
 };
 
-// ---------------------------------------------------------------------------------------------
-// Tap tables.  One thread per (RoI, axis, bin): the bin's g samples give up to 2g (pixel, weight)
-// taps; equal pixels are merged (weights summed in sample order); unused slots are marked empty.
-// Layout: taps[k][PH + PW bins][2g slots]; y bins first.  Invalid samples (outside [-1, n], reading
-// S6) produce no tap, so the product Y x X enumerates exactly the valid samples of the forward.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void pull_taps_item(const LevelsParam& lv, const RoiArgs& a, int64_t idx,
-                                               PullTap* __restrict__ taps) {
-  const int nb = a.PH + a.PW;
-  const int k = (int)(idx / nb), b = (int)(idx - (int64_t)k * nb);
-  const bool isy = b < a.PH;
-  const int bin = isy ? b : b - a.PH;
-  const int g = a.sampling_ratio, slots = 2 * g;
-  const float* r = a.rois + 5 * (int64_t)k;
-  const float x1 = __ldg(r + 1), y1 = __ldg(r + 2), x2 = __ldg(r + 3), y2 = __ldg(r + 4);
-  const int level = level_of(x1, y1, x2, y2, lv.L, a.finest_scale);
-  const RoiGeom geo = roi_geom(x1, y1, x2, y2, lv.scale[level], a.PH, a.PW, g, a.aligned);
-  const int n = isy ? lv.h[level] : lv.w[level];
-  const float scale_w = isy ? geo.inv_count : 1.0f;
-  const float start = isy ? geo.sy : geo.sx, bsz = isy ? geo.bh : geo.bw;
-  PullTap* out = taps + idx * slots;
-  const uint32_t tag = (uint32_t)bin << 24;
-  if (g <= 2) {   // the usual case: merge in registers, one 8-byte store per slot
-    uint32_t pix[4] = {kPixMask, kPixMask, kPixMask, kPixMask};
-    float w[4] = {0.f, 0.f, 0.f, 0.f};
-    int cnt = 0;
-    auto add = [&](uint32_t p, float v) {
-      bool found = false;
-#pragma unroll
-      for (int q = 0; q < 4; ++q)
-        if (q < cnt && pix[q] == p) { w[q] += v; found = true; }
-      if (!found) {
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-          if (q == cnt) { pix[q] = p; w[q] = v; }
-        ++cnt;
-      }
-    };
-    for (int i = 0; i < g; ++i) {
-      const AxisTap t = axis_tap(sample_coord(start, bsz, bin, i, g), n);
-      if (!t.valid) continue;
-      add((uint32_t)t.lo, t.wh * scale_w);
-      add((uint32_t)t.hi, t.wl * scale_w);
-    }
-#pragma unroll
-    for (int q = 0; q < 4; ++q)
-      if (q < slots) { PullTap e; e.pb = tag | pix[q]; e.w = w[q]; out[q] = e; }
-    return;
-  }
-  int cnt = 0;
-  auto add = [&](int pix, float w) {
-    for (int q = 0; q < cnt; ++q)
-      if ((out[q].pb & kPixMask) == (uint32_t)pix) { out[q].w += w; return; }
-    out[cnt].pb = tag | (uint32_t)pix;
-    out[cnt].w = w;
-    ++cnt;
-  };
-  for (int i = 0; i < g; ++i) {
-    const AxisTap t = axis_tap(sample_coord(start, bsz, bin, i, g), n);
-    if (!t.valid) continue;
-    add(t.lo, t.wh * scale_w);
-    add(t.hi, t.wl * scale_w);
-  }
-  for (int q = cnt; q < slots; ++q) { out[q].pb = tag | kPixMask; out[q].w = 0.0f; }
-}
-
-constexpr int kPrepThreads = 256;
-constexpr int kPrepWarps = kPrepThreads / 32;
-
-// ---------------------------------------------------------------------------------------------
-// Stable bucketing by (level, image): key = level * N + batch_idx.  Feeds the pull backward
-// (raf_backward_pull.cu), whose tiles walk the RoIs of their own (level, image) in ascending k --
-// a fixed order, hence bit-reproducible sums.  RoIs with an invalid batch index are dropped.
-//   bperm[K]      RoI indices grouped by key, ascending k inside a key
-//   boff[NK + 1]  start of every key's group (NK = L * N)
-//   bwin[K]       (optional) in bperm order: conservative window {ymin, ymax, xmin, xmax} of the
-//                 pixels the RoI's samples can touch on its level (empty: ymin > ymax)
-// Block 0 of pull_prep_kernel (the other blocks write the tap tables, same launch): 8 warps; warp w owns the contiguous RoI range [w*q, (w+1)*q).  cnt[w][key] first
-// counts, then (after a scan over keys, warps minor) holds the next free slot of (key, warp):
-// warp-private rows, so neither atomics nor block barriers inside the walks.
-// ---------------------------------------------------------------------------------------------
-
-// Pixels an axis can touch: samples are monotone in (bin, i) up to rounding, so the first and the
-// last sample (with slack for that rounding) bound all of them; a sample at v touches
-// floor(max(v,0)) and the next pixel (clamped to n-1); samples outside [-1, n] touch nothing.
-__device__ __forceinline__ void axis_window(float start, float bin, int P, int g, int n, int& lo, int& hi) {
-  const float va = sample_coord(start, bin, 0, 0, g), vb = sample_coord(start, bin, P - 1, g - 1, g);
-  const float slack = 0.01f + 1e-6f * fmaxf(fabsf(va), fabsf(vb));
-  const float vlo = fminf(va, vb) - slack, vhi = fmaxf(va, vb) + slack;
-  lo = 0x7fffffff; hi = -1;
-  if (!(vlo <= vhi) || vhi < -1.0f || vlo > (float)n) return;   // NaN or entirely outside
-  lo = (int)fminf(fmaxf(vlo, 0.0f), (float)(n - 1));
-  hi = min(n - 1, (int)fminf(fmaxf(vhi, 0.0f), (float)(n - 1)) + 1);
-}
-
 __global__ void __launch_bounds__(kPrepThreads, 1)
-pull_prep_kernel(const LevelsParam lv, const RoiArgs a, int32_t* __restrict__ bperm,
-                 int32_t* __restrict__ boff, int4* __restrict__ bwin, PullTap* __restrict__ taps) {
-  extern __shared__ int s_cnt[];  // [kPrepWarps][NK + 1] then [NK + 1] totals/offsets
-  if (blockIdx.x > 0) {           // blocks 1.. : tap tables (independent of the bucketing)
-    const int64_t idx = (int64_t)(blockIdx.x - 1) * kPrepThreads + threadIdx.x;
-    if (idx < (int64_t)a.K * (a.PH + a.PW)) pull_taps_item(lv, a, idx, taps);
-    return;
-  }
-  const int K = a.K, L = lv.L, N = lv.n;
-  const int NK = L * N, NK1 = NK + 1;
-  int* s_tot = s_cnt + kPrepWarps * NK1;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int q = ((K + kPrepWarps - 1) / kPrepWarps + 31) & ~31;  // per-warp range, multiple of 32
-  const int lo = warp * q, hi = min(K, lo + q);
-  for (int i = tid; i < kPrepWarps * NK1 + NK1; i += kPrepThreads) s_cnt[i] = 0;
-  __syncthreads();
-
-  auto key_of = [&](int k) -> int {
-    if (k >= hi) return -1;
-    const float* r = a.rois + 5 * (int64_t)k;
-    const int b = batch_index_of(r[0], N);
-    if (b < 0) return NK;  // dropped
-    return level_of(r[1], r[2], r[3], r[4], L, a.finest_scale) * N + b;
-  };
-
-  int* mine = s_cnt + warp * NK1;
-  for (int k0 = lo; k0 < hi; k0 += 32) {
-    const int key = key_of(k0 + lane);
-    const unsigned peers = __match_any_sync(0xffffffffu, key);
-    if (key >= 0 && lane == __ffs(peers) - 1) mine[key] += __popc(peers);
-    __syncwarp();
-  }
-  __syncthreads();
-
-  // totals per key
-  for (int key = tid; key < NK1; key += kPrepThreads) {
-    int t = 0;
-    for (int w = 0; w < kPrepWarps; ++w) t += s_cnt[w * NK1 + key];
-    s_tot[key] = t;
-  }
-  __syncthreads();
-  if (warp == 0) {  // exclusive scan of the totals over keys, 32 at a time
-    int carry = 0;
-    for (int base = 0; base < NK1; base += 32) {
-      const int key = base + lane;
-      const int v = key < NK1 ? s_tot[key] : 0;
-      int incl = v;
-      for (int d = 1; d < 32; d <<= 1) {
-        const int o = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += o;
-      }
-      if (key < NK1) s_tot[key] = carry + incl - v;
-      carry += __shfl_sync(0xffffffffu, incl, 31);
-    }
-  }
-  __syncthreads();
-  for (int key = tid; key < NK1; key += kPrepThreads) {
-    if (key <= NK) boff[key] = s_tot[key];  // boff[NK] = number of kept RoIs
-    int run = s_tot[key];
-    for (int w = 0; w < kPrepWarps; ++w) {
-      const int c = s_cnt[w * NK1 + key];
-      s_cnt[w * NK1 + key] = run;
-      run += c;
-    }
-  }
-  __syncthreads();
-
-  for (int k0 = lo; k0 < hi; k0 += 32) {
-    const int k = k0 + lane;
-    const int key = key_of(k);
-    const unsigned peers = __match_any_sync(0xffffffffu, key);
-    const int base = (key >= 0) ? mine[key] : 0;
-    __syncwarp();
-    if (key >= 0 && key < NK) {
-      const int p = base + __popc(peers & ((1u << lane) - 1u));
-      bperm[p] = k;
-      if (bwin) {
-        const float* r = a.rois + 5 * (int64_t)k;
-        const int level = key / N;
-        const RoiGeom geo = roi_geom(r[1], r[2], r[3], r[4], lv.scale[level], a.PH, a.PW, a.sampling_ratio, a.aligned);
-        int4 w;
-        axis_window(geo.sy, geo.bh, a.PH, a.sampling_ratio, lv.h[level], w.x, w.y);
-        axis_window(geo.sx, geo.bw, a.PW, a.sampling_ratio, lv.w[level], w.z, w.w);
-        if (w.x > w.y || w.z > w.w) w = make_int4(0x7fffffff, -1, 0x7fffffff, -1);
-        bwin[p] = w;
-      }
-    }
-    if (key >= 0 && lane == __ffs(peers) - 1) mine[key] = base + __popc(peers);
-    __syncwarp();
-  }
+pull_prep_kernel(const LevelsParam lv, const RoiArgs a, const PullPrepOut o) {
+  extern __shared__ int s_prep[];
+  pull_prep_block(lv, a, o, (int)blockIdx.x, s_prep);
 }
 
-size_t bucket_smem_bytes(int L, int N) { return (size_t)(kPrepWarps + 1) * ((size_t)L * N + 1) * sizeof(int); }
+size_t bucket_smem_bytes(int L, int N) { return (size_t)(kPrepThreads / 32 + 1) * ((size_t)L * N + 1) * sizeof(int); }
 
 int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, int32_t* boff, int4* bwin,
                      PullTap* taps, cudaStream_t stream) {
@@ -244,9 +62,8 @@ int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, in
   if (smem > 48 * 1024 &&
       cudaFuncSetAttribute(pull_prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return RAF_ERR_CUDA;
-  const int64_t items = (int64_t)a.K * (a.PH + a.PW);
-  const unsigned blocks = 1 + (unsigned)((items + kPrepThreads - 1) / kPrepThreads);
-  pull_prep_kernel<<<blocks, kPrepThreads, smem, stream>>>(lv, a, bperm, boff, bwin, taps);
+  const PullPrepOut o{bperm, boff, bwin, taps, pull_prep_blocks(a, kPrepThreads)};
+  pull_prep_kernel<<<(unsigned)o.nblocks, kPrepThreads, smem, stream>>>(lv, a, o);
   count_launch();
   return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;
 }

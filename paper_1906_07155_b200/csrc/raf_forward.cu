@@ -15,6 +15,7 @@
 //  * fwd_generic_kernel  any strides / any C / adaptive sampling: one thread per output element.
 #include "raf_device.cuh"
 #include "raf_host.h"
+#include "raf_pull_prep.cuh"
 
 namespace raf {
 
@@ -113,7 +114,7 @@ __device__ __forceinline__ void fwd_dispatch_x(int nx, const T* rp0, const T* rp
 template <typename T>
 __global__ void __launch_bounds__(32 * kFwdWarps, 3)
 fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
-              int64_t os_w, int chunks) {
+              int64_t os_w, int chunks, const PullPrepOut prep) {
   using V = Vec16<T>;
   constexpr int VN = V::N;
   extern __shared__ __align__(16) unsigned char fwd_smem[];
@@ -123,7 +124,12 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   int* s_cnt = reinterpret_cast<int*>(s_tab + nb * slots);     // [PH + PW]
   __shared__ int s_b;
 
-  const int k = blockIdx.x / chunks, chunk = blockIdx.x - k * chunks;
+  if ((int)blockIdx.x < prep.nblocks) {   // leading blocks: the backward's prep tables (same RoIs, same
+    pull_prep_block(lv, a, prep, (int)blockIdx.x, reinterpret_cast<int*>(fwd_smem));   // geometry), for free
+    return;
+  }
+  const int bid = (int)blockIdx.x - prep.nblocks;
+  const int k = bid / chunks, chunk = bid - k * chunks;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   const float* r = a.rois + 5 * (int64_t)k;
   const float r0 = __ldg(r), x1 = __ldg(r + 1), y1 = __ldg(r + 2), x2 = __ldg(r + 3), y2 = __ldg(r + 4);
@@ -241,18 +247,32 @@ fwd_generic_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, i
 
 template <typename T>
 static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, const int64_t* os,
-                         bool channels_last, cudaStream_t stream) {
+                         bool channels_last, const PullPrepOut* prep, cudaStream_t stream) {
   T* o = reinterpret_cast<T*>(out);
   const int g = a.sampling_ratio;
   if (channels_last && g > 0) {
     const int CV = lv.c / Vec16<T>::N;
     const int chunks = (CV + 31) / 32;
-    const size_t smem = (size_t)(a.PH + a.PW) * (2 * g * sizeof(FwdTap) + sizeof(int));
+    size_t smem = (size_t)(a.PH + a.PW) * (2 * g * sizeof(FwdTap) + sizeof(int));
     int nw = a.PH < kFwdWarps ? a.PH : kFwdWarps;          // one warp per output bin row
     while (32 * nw < a.PH + a.PW) ++nw;                     // the table set-up needs PH + PW threads
-    fwd_cl_kernel<T><<<(unsigned)((int64_t)a.K * chunks), 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2], os[3],
-                                                                                          chunks);
+    PullPrepOut po{nullptr, nullptr, nullptr, nullptr, 0};
+    if (prep) {                                             // carry the backward's prep in the leading blocks
+      po = *prep;
+      po.nblocks = pull_prep_blocks(a, 32 * nw);
+      const size_t psmem = (size_t)(nw + 1) * ((size_t)lv.L * lv.n + 1) * sizeof(int);
+      if (psmem > smem) smem = psmem;
+    }
+    if (smem > 48 * 1024 &&
+        cudaFuncSetAttribute(fwd_cl_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      return RAF_ERR_CUDA;
+    fwd_cl_kernel<T><<<(unsigned)((int64_t)a.K * chunks + po.nblocks), 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2],
+                                                                                               os[3], chunks, po);
   } else {
+    if (prep) {   // generic path: the prep tables still get written, by their own launch
+      const int rc = launch_pull_prep(lv, a, prep->bperm, prep->boff, prep->bwin, prep->taps, stream);
+      if (rc) return rc;
+    }
     const int64_t total = (int64_t)a.K * lv.c * a.PH * a.PW;
     const int64_t blocks = (total + 255) / 256;
     const int grid = (int)(blocks < (int64_t)148 * 64 ? blocks : (int64_t)148 * 64);
@@ -263,11 +283,11 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
 }
 
 int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
-                   const int64_t* out_strides, bool channels_last, cudaStream_t stream) {
+                   const int64_t* out_strides, bool channels_last, const PullPrepOut* prep, cudaStream_t stream) {
   switch (dtype) {
-    case RAF_F32: return forward_typed<float>(lv, a, out, out_strides, channels_last, stream);
-    case RAF_F16: return forward_typed<__half>(lv, a, out, out_strides, channels_last, stream);
-    case RAF_BF16: return forward_typed<__nv_bfloat16>(lv, a, out, out_strides, channels_last, stream);
+    case RAF_F32: return forward_typed<float>(lv, a, out, out_strides, channels_last, prep, stream);
+    case RAF_F16: return forward_typed<__half>(lv, a, out, out_strides, channels_last, prep, stream);
+    case RAF_BF16: return forward_typed<__nv_bfloat16>(lv, a, out, out_strides, channels_last, prep, stream);
   }
   return RAF_ERR_DTYPE;
 }

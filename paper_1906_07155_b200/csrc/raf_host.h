@@ -26,8 +26,11 @@ int launch_assign_levels(const float* rois, int K, int L, float finest_scale, in
 
 // Forward.  `channels_last` = every level has sc == 1 and the output has stride 1 along C, with
 // 16-byte aligned pixel vectors (checked by the caller).
+struct PullPrepOut;
+// `prep` (may be null): also write the pull backward's prep tables (see launch_pull_prep) -- in the
+// channels-last path they ride in the leading blocks of the forward launch.
 int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
-                   const int64_t* out_strides, bool channels_last, cudaStream_t stream);
+                   const int64_t* out_strides, bool channels_last, const PullPrepOut* prep, cudaStream_t stream);
 
 // Backward (atomic scatter).  The gradient pyramid must already hold its starting values.
 int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a,

@@ -243,6 +243,38 @@ def test_backward_pull_unsupported_sizes_fall_back():
     assert e.value.status == -5
 
 
+@pytest.mark.parametrize("layout_fwd", ["cl", "nchw"])
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_backward_reuses_prep_written_by_forward(layout_fwd, dtype):
+    """RAF_REUSE_PREP: the forward call leaves the RoI buckets / tap tables in the workspace (in the
+    leading blocks of its own launch for channels-last, by a separate launch otherwise); the backward
+    skips its prep launch.  Result must equal the oracle and the stand-alone backward bit for bit."""
+    wl = inputs.make_workload(5, n_img=3, per_img=120, channels=64)
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    feats, _ = T.device_feats(wl.feats, dtype, layout_fwd)
+    rois = torch.from_numpy(wl.rois).cuda()
+    go_t = torch.from_numpy(wl.grad_out).to(T.TORCH_DTYPE[dtype])
+    go = T.to_layout(go_t.cuda(), "cl")
+    ws = T.workspace(K, L, PH, PW, 2)
+    ws.fill_(0xAB)
+    out = T.empty_layout((K, C, PH, PW), feats[0].dtype, layout_fwd)
+    B.roi_align_fpn_forward(feats, cfg.scales, rois, out, 2, True, cfg.finest_scale, ws)
+    g1 = [T.empty_layout(s, torch.float32, "cl", fill=float("nan")) for s in cfg.level_shapes]
+    B.roi_align_fpn_backward(g1, cfg.scales, go, rois, 2, True, cfg.finest_scale, B.RAF_REUSE_PREP, ws)
+    torch.cuda.synchronize()
+    ws2 = T.workspace(K, L, PH, PW, 2)
+    g2 = [T.empty_layout(s, torch.float32, "cl", fill=float("nan")) for s in cfg.level_shapes]
+    B.roi_align_fpn_backward(g2, cfg.scales, go, rois, 2, True, cfg.finest_scale, 0, ws2)
+    torch.cuda.synchronize()
+    for a_, b_ in zip(g1, g2):
+        assert torch.equal(a_, b_)
+    ref, S = R.backward(cfg.level_shapes, cfg.scales, go_t.to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
+                        cfg.finest_scale)
+    T.assert_backward_close([t.to(torch.float64).cpu().numpy() for t in g1], ref, S)
+
+
 def test_backward_degenerate_and_invalid_rois():
     wl = inputs.make_workload(2, n_img=2, per_img=8, channels=16)
     wl.rois = np.array([[0, 100, 100, 100, 100], [1, 300, 200, 100, 50], [0, -500, -500, -400, -400],

@@ -284,6 +284,15 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
 
 int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
                    const int64_t* out_strides, bool channels_last, const PullPrepOut* prep, cudaStream_t stream) {
+#ifdef RAF_FWD_TMA
+  if (channels_last) {   // bulk-async staged variant (raf_forward_tma.cu) where it applies
+    int rc = launch_forward_tma(lv, dtype, a, out, out_strides, stream);
+    if (rc != RAF_ERR_UNSUPPORTED) {
+      if (rc == RAF_OK && prep) rc = launch_pull_prep(lv, a, prep->bperm, prep->boff, prep->bwin, prep->taps, stream);
+      return rc;
+    }
+  }
+#endif
   switch (dtype) {
     case RAF_F32: return forward_typed<float>(lv, a, out, out_strides, channels_last, prep, stream);
     case RAF_F16: return forward_typed<__half>(lv, a, out, out_strides, channels_last, prep, stream);

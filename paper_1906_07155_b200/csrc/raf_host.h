@@ -32,6 +32,10 @@ struct PullPrepOut;
 int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
                    const int64_t* out_strides, bool channels_last, const PullPrepOut* prep, cudaStream_t stream);
 
+// Forward, bulk-async (TMA) staged variant; RAF_ERR_UNSUPPORTED when the arguments are outside its range.
+int launch_forward_tma(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
+                       const int64_t* out_strides, cudaStream_t stream);
+
 // Backward (atomic scatter).  The gradient pyramid must already hold its starting values.
 int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a,
                            const void* grad_out, const int64_t* gout_strides, bool channels_last,

@@ -374,3 +374,52 @@ def test_host_entry_points_match_device_path():
     torch.cuda.synchronize()
     ref_g, S = R.backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, (7, 7), 2, True, 56.0)
     T.assert_backward_close([g.numpy().astype(np.float64) for g in grads_h], ref_g, S)
+
+
+# ------------------------------------------------------------------------------------------------
+# guard bands (compute-sanitizer is closed on this GPU pool): every buffer the library writes sits
+# inside a larger sentinel-filled allocation; the margins must come back untouched
+# ------------------------------------------------------------------------------------------------
+def _guarded(nbytes, margin=4096):
+    buf = torch.full((nbytes + 2 * margin,), 0x5A, dtype=torch.uint8, device="cuda")
+    return buf, buf[margin:margin + nbytes]
+
+
+def _margins_intact(buf, nbytes, margin=4096):
+    return bool((buf[:margin] == 0x5A).all()) and bool((buf[margin + nbytes:] == 0x5A).all())
+
+
+@pytest.mark.parametrize("index,dtype,kw,P", [
+    (2, "f32", dict(n_img=2, per_img=150, channels=64), (7, 7)),
+    (5, "bf16", dict(n_img=2, per_img=100, channels=40), (7, 7)),     # boxes partly outside, partial chunk
+    (4, "f16", dict(n_img=1, per_img=60, channels=264), (14, 14)),
+])
+@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC, B.RAF_REUSE_PREP])
+def test_no_out_of_bounds_writes(index, dtype, kw, P, flags):
+    wl = inputs.make_workload(index, **kw)
+    cfg = wl.cfg
+    tdt = T.TORCH_DTYPE[dtype]
+    esz = 4 if dtype == "f32" else 2
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    PH, PW = P
+    feats, _ = T.device_feats(wl.feats, dtype, "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    n_out = K * C * PH * PW
+    obuf, oview = _guarded(n_out * esz)
+    out = oview.view(tdt).view(K, PH, PW, C).permute(0, 3, 1, 2)
+    wsz = B.roi_align_fpn_workspace_bytes(K, L, PH, PW, 2, flags)
+    wbuf, ws = _guarded(wsz)
+    B.roi_align_fpn_forward(feats, cfg.scales, rois, out, 2, True, cfg.finest_scale, ws)
+    gbufs, grads = [], []
+    for (n, c, h, w) in cfg.level_shapes:
+        gb, gv = _guarded(n * c * h * w * 4)
+        gbufs.append((gb, n * c * h * w * 4))
+        grads.append(gv.view(torch.float32).view(n, h, w, c).permute(0, 3, 1, 2))
+    gout = T.to_layout(torch.randn((K, C, PH, PW), device="cuda").to(tdt), "cl")
+    B.roi_align_fpn_backward(grads, cfg.scales, gout, rois, 2, True, cfg.finest_scale, flags, ws)
+    torch.cuda.synchronize()
+    assert _margins_intact(obuf, n_out * esz), "forward wrote outside its output"
+    assert _margins_intact(wbuf, wsz), "workspace overrun"
+    for gb, nb in gbufs:
+        assert _margins_intact(gb, nb), "backward wrote outside the gradient pyramid"
+    assert all(torch.isfinite(g).all() for g in grads) and torch.isfinite(out.float()).all()

@@ -373,8 +373,14 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
   for (int i = 0; i < lv.L; ++i) {
     const int l = lv.L - 1 - i;  // coarsest level first
     t.order[i] = l;
-    int th = kTH;                // aim for >= 128 tiles per level and image
-    while (th > 1 && (int64_t)lv.h[l] * lv.w[l] < (int64_t)128 * th * kTW) th >>= 1;
+#ifndef RAF_PULL_MINTILES
+#define RAF_PULL_MINTILES 64
+#endif
+#ifndef RAF_PULL_MAXTH
+#define RAF_PULL_MAXTH kTH
+#endif
+    int th = RAF_PULL_MAXTH;     // aim for >= RAF_PULL_MINTILES tiles per level and image
+    while (th > 1 && (int64_t)lv.h[l] * lv.w[l] < (int64_t)RAF_PULL_MINTILES * th * kTW) th >>= 1;
     t.th[l] = th;
     t.tiles_y[l] = (lv.h[l] + th - 1) / th;
     t.tiles_x[l] = (lv.w[l] + kTW - 1) / kTW;

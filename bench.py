@@ -314,7 +314,8 @@ def run_ours(args):
     ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz)
     peak, peak_src = peaks()
     from paper_1906_07155_b200 import ncu_traffic
-    traffic = ncu_traffic.TRAFFIC_BYTES.get(args.config, {}) if args.layout == "cl" and args.backward == "auto" else {}
+    traffic = (ncu_traffic.TRAFFIC_BYTES.get(args.config, {})
+               if args.layout == "cl" and args.backward == "auto" and not args.no_reuse_prep else {})
     legs = {"fwd": (ab["fwd"], fwd_ms)}
     if bwd_ms is not None:
         legs["bwd"] = (ab["bwd"], bwd_ms)

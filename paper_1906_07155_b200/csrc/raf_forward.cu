@@ -26,6 +26,9 @@ struct FwdTap {
   float w;
 };
 
+#ifndef RAF_FWD_MINB
+#define RAF_FWD_MINB 3
+#endif
 constexpr int kFwdWarps = 8;   // max warps per CTA (one output bin row each, strided)
 
 // Merged taps of bin `bin` of one axis into tab[0..2g) (shared memory); returns the count.
@@ -112,7 +115,7 @@ __device__ __forceinline__ void fwd_dispatch_x(int nx, const T* rp0, const T* rp
 // Channels-last forward.  CTA = (RoI, chunk of 32 channel-vectors); warp = output bin row(s);
 // lanes = channel vectors (16 bytes each: a warp-wide load covers 512 contiguous bytes).
 template <typename T>
-__global__ void __launch_bounds__(32 * kFwdWarps, 3)
+__global__ void __launch_bounds__(32 * kFwdWarps, RAF_FWD_MINB)
 fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
               int64_t os_w, int chunks, const PullPrepOut prep) {
   using V = Vec16<T>;

@@ -327,7 +327,8 @@ def run_ours(args):
         return {"bound": "hbm", "kernel": name, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": traffic.get(name), "traffic_source": traffic.get("source"), "algorithmic_bytes": by, "ms": ms,
                 "peak_source": peak_src,
-                "note": "ms = CUDA-event time of the whole C-ABI call of this leg (bwd: prep launch + pull kernel)"}
+                "note": "ms = CUDA-event time of the whole C-ABI call of this leg (fwd: gather kernel incl. the "
+                        "backward's prep blocks under RAF_REUSE_PREP; bwd: pull kernel, + its prep launch otherwise)"}
 
     step_ms = total_ms / args.steps
     step_bytes = ab["fwd"] + (ab["bwd"] if cfg.backward else 0)

@@ -9,7 +9,7 @@
 //                        reduction `red.global.add.v4.f32` (north_star), a warp covers 512 B.
 //  * bwd_generic_kernel  any strides / adaptive sampling: scalar atomicAdd per tap.
 // Summation order across RoIs is whatever the L2 atomics see (several results are correct;
-// tolerance reading S11).  The deterministic variant lives in raf_backward_det.cu.
+// tolerance reading S11).  The deterministic pull variant (the default) lives in raf_backward_pull.cu.
 #include "raf_device.cuh"
 #include "raf_host.h"
 

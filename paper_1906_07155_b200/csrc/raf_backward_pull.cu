@@ -12,21 +12,29 @@
 //   g[y][x] += sum_{(ph,wy) in Y_k(y)} sum_{(pw,wx) in X_k(x)}  wy * wx * gout[k][ph][pw]
 // where Y_k(y) lists the output-bin rows with a sample tap on pixel row y (weights of the same
 // bin and pixel merged, 1/count folded in) and X_k(x) likewise for columns.  Those per-RoI, per-axis
-// TAP TABLES are built once per call by pull_taps_kernel (same canonical fp32 coordinates and
-// weights as the forward, raf_device.cuh) and live in the workspace (L2 resident: 448 B per RoI).
+// TAP TABLES are built once per call by the prep blocks (raf_pull_prep.cuh: same canonical fp32
+// coordinates and weights as the forward) and live in the workspace (L2 resident: 448 B per RoI).
+// The prep work -- stable (level, image) bucketing, a conservative pixel window per RoI, the tap
+// tables -- runs either as pull_prep_kernel or, with RAF_REUSE_PREP, in the leading blocks of the
+// forward launch.
 //
-// bwd_pull_kernel, per tile:
-//  (A) scan the bucket's RoI windows (bwin, written in bucket order by bucket_rois_kernel) and keep
-//      the RoIs whose window meets the tile (ballot compaction, order preserved);
-//  (B) for up to 64 candidates at a time, one warp per candidate holds the RoI's taps in its lanes
-//      and ballots them against the tile's 8 rows and 8 columns: shared memory gets, per (candidate,
-//      row) and (candidate, column), the first entry (bin, weight) + the entry count, and the ballot
-//      masks for the (rarer) further entries;
-//  (C) every warp owns one pixel row; it walks its 8 pixels one at a time, lanes spread over the
-//      256 channels (two float4 accumulators per lane), and for every candidate reads two uniform
-//      8-byte table entries: no entry on the row or on the column -> next candidate; otherwise
-//      acc += wy * wx * gout[k][ph][pw][channels] with 128-bit loads.  One pixel = 8 registers of
-//      state, so ~40 warps per SM hide the L2 latency of first-touch grad_out lines.
+// bwd_pull_kernel, per tile (TH x 8 pixels, TH = 8 on large levels, smaller on small dense ones):
+//  (A) 256 threads test 512 bucket windows (bwin, bucket order) against the tile in one round trip
+//      and keep the RoIs that meet it (ballot compaction, order preserved);
+//  (B) per pass of <= 16 candidates, one warp per candidate holds the RoI's taps in its lanes and
+//      ballots them against the tile's rows and columns: shared memory gets, per (candidate, row)
+//      and (candidate, column), the first two entries (premultiplied grad_out offset, weight) + the
+//      entry count, and the ballot masks for the (rarer) further entries; then, lanes = pixels, the
+//      row x column entries of every pixel are expanded into <= 4 (offset, wy*wx) PAIRS per
+//      (pixel, candidate) and their number;
+//  (C) warp w owns pixel (i, (w + i) % 8) of every tile row i (one pixel per row and column: the
+//      warps of a CTA carry about the same load); one pixel at a time, lanes spread over the 256
+//      channels (two float4 accumulators per lane = 8 registers of state, 64 registers total, 4
+//      CTAs per SM): a ballot over the pair counts gives the candidates that hit the pixel; each
+//      hit = one or two 16-byte shared loads + two 128-bit grad_out loads + 8 FFMA per pair.
+//      Candidates with more than two entries on an axis (bins narrower than half a pixel) walk the
+//      ballot masks instead (exact).  Tiles with more than 16 candidates take several passes, the
+//      partial sums parked in the gradient tensor itself.
 // Tiles of the coarsest level are scheduled first (most RoIs per pixel).
 #include "raf_device.cuh"
 #include "raf_host.h"

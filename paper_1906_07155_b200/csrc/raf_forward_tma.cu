@@ -17,17 +17,17 @@
 //
 // STATUS (round 1): EXPERIMENTAL, compiled always but dispatched only when the library is built
 // with -DRAF_FWD_TMA (RAF_FWD_TMA=1 python -m paper_1906_07155_b200.build).  Parity-green under that
-// build (tests/test_gpu_parity.py forward cases), but 3-4x SLOWER than the direct kernel on config 2
-// (profiles/r1_experiments.md): the 12-row ring is shallower than one RoI window, so table building,
-// copy issue and consumption serialise per item, and 512-byte copies are too small for the copy
-// engine.  Round-2 work: table builder and loader in separate warps running items ahead, one 2-D
-// tensor-map copy per row band, tap tables in registers.
+// build (all forward cases of tests/test_gpu_parity.py), but 2.5x SLOWER than the direct kernel on
+// config 2 (fp32 167 us, bf16 92 us vs 57 / 39 us; profiles/r1_experiments.md).  Two persistent
+// CTAs per SM with a 6-row ring each: every item is latency-bound row by row, and shared memory
+// (~200 KB per SM) cannot hold more bytes in flight than the register file already does for the
+// direct kernel (~118 KB per SM), so staging buys no extra memory-level parallelism here.
 #include "raf_device.cuh"
 #include "raf_host.h"
 
 namespace raf {
 
-constexpr int kTmaSlots = 12;          // ring of pixel-row slots
+constexpr int kTmaSlots = 6;           // ring of pixel-row slots (two CTAs per SM)
 constexpr int kTmaSlotPx = 32;         // pixels per slot (window width limit of the staged path)
 constexpr int kTmaChunkBytes = 512;    // channel bytes per pixel and work item
 constexpr int kTmaMaxBins = 16;        // PH, PW <= 16 in this variant
@@ -222,6 +222,42 @@ __device__ __forceinline__ void tma_build_tables(const LevelsParam& lv, const Ro
   __syncwarp();
 }
 
+// acc += sum_{a < NY, b < NX} (yw[a] * xw[b]) * row_a[xo[b]]: every 16-byte shared load is issued
+// before the first use.  rp[a] already includes the lane's 16-byte offset; xo[b] = pixel * 512 bytes.
+template <typename T, int NY, int NX>
+__device__ __forceinline__ void tma_accumulate(const unsigned char* const (&rp)[4], const float (&yw)[4],
+                                               const int (&xo)[4], const float (&xw)[4],
+                                               float (&acc)[Cvt16<T>::N]) {
+  constexpr int VN = Cvt16<T>::N;
+  uint4 raw[NY][NX];
+#pragma unroll
+  for (int a = 0; a < NY; ++a)
+#pragma unroll
+    for (int b = 0; b < NX; ++b) raw[a][b] = *reinterpret_cast<const uint4*>(rp[a] + xo[b]);
+#pragma unroll
+  for (int a = 0; a < NY; ++a)
+#pragma unroll
+    for (int b = 0; b < NX; ++b) {
+      float v[VN];
+      Cvt16<T>::widen(raw[a][b], v);
+      const float w = yw[a] * xw[b];
+#pragma unroll
+      for (int j = 0; j < VN; ++j) acc[j] = fmaf(w, v[j], acc[j]);
+    }
+}
+
+template <typename T, int NY>
+__device__ __forceinline__ void tma_dispatch_x(int nx, const unsigned char* const (&rp)[4], const float (&yw)[4],
+                                               const int (&xo)[4], const float (&xw)[4],
+                                               float (&acc)[Cvt16<T>::N]) {
+  switch (nx) {
+    case 1: tma_accumulate<T, NY, 1>(rp, yw, xo, xw, acc); break;
+    case 2: tma_accumulate<T, NY, 2>(rp, yw, xo, xw, acc); break;
+    case 3: tma_accumulate<T, NY, 3>(rp, yw, xo, xw, acc); break;
+    default: tma_accumulate<T, NY, 4>(rp, yw, xo, xw, acc); break;
+  }
+}
+
 struct TmaSmem {   // dynamic shared memory carve-up (ring first: 128-byte aligned slots)
   static constexpr int kSlotBytes = kTmaSlotPx * kTmaChunkBytes;
   unsigned char ring[kTmaSlots][kSlotBytes];
@@ -232,7 +268,7 @@ struct TmaSmem {   // dynamic shared memory carve-up (ring first: 128-byte align
 };
 
 template <typename T>
-__global__ void __launch_bounds__(kTmaThreads, 1)
+__global__ void __launch_bounds__(kTmaThreads, 2)
 fwd_tma_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
                int64_t os_w, int chunks) {
   constexpr int VN = Cvt16<T>::N;
@@ -315,12 +351,32 @@ fwd_tma_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64
             ++waited;
           }
         }
+        const unsigned char* rp[4];
+        float yw[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {   // y taps of this bin row: row pointers (lane's 16 bytes) and weights
+          const int sl = (staged && q < ny) ? (int)((g0 + Tb.yseq[ph][q]) % kTmaSlots) : 0;
+          rp[q] = &S.ring[sl][lane * 16];
+          yw[q] = Tb.ytap[ph][q].w;
+        }
         for (int pw = cw; pw < PW; pw += kTmaConsumers) {
           const int nx = Tb.xcnt[pw];
           float acc[VN];
 #pragma unroll
           for (int j = 0; j < VN; ++j) acc[j] = 0.0f;
-          if (act) {
+          if (act && staged && ny > 0 && nx > 0) {
+            int xo[4];
+            float xw[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) { const TmaTap e = Tb.xtap[pw][q]; xo[q] = e.pix * kTmaChunkBytes; xw[q] = e.w; }
+            switch (ny) {
+              case 1: tma_dispatch_x<T, 1>(nx, rp, yw, xo, xw, acc); break;
+              case 2: tma_dispatch_x<T, 2>(nx, rp, yw, xo, xw, acc); break;
+              case 3: tma_dispatch_x<T, 3>(nx, rp, yw, xo, xw, acc); break;
+              default: tma_dispatch_x<T, 4>(nx, rp, yw, xo, xw, acc); break;
+            }
+            Vec16<T>::store(out_k + ph * os_h + pw * os_w, acc);
+          } else if (act) {
             for (int qa = 0; qa < ny; ++qa) {
               const TmaTap ey = Tb.ytap[ph][qa];
               const unsigned char* srow = staged ? &S.ring[(g0 + Tb.yseq[ph][qa]) % kTmaSlots][lane * 16] : nullptr;
@@ -371,7 +427,7 @@ static int forward_tma_typed(const LevelsParam& lv, const RoiArgs& a, void* out,
   if (cudaFuncSetAttribute(fwd_tma_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return RAF_ERR_CUDA;
   const int64_t items = (int64_t)a.K * chunks;
-  const unsigned grid = (unsigned)(items < sm_count ? items : sm_count);
+  const unsigned grid = (unsigned)(items < 2 * sm_count ? items : 2 * sm_count);
   fwd_tma_kernel<T><<<grid, kTmaThreads, smem, stream>>>(lv, a, reinterpret_cast<T*>(out), os[0], os[2], os[3], chunks);
   count_launch();
   return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;

@@ -330,6 +330,47 @@ def test_backward_full_size_config2(flags):
         assert np.all(g[np.broadcast_to(m[:, None] == 0, g.shape)] == 0)
 
 
+@pytest.mark.parametrize("index", [2, 4, 5])
+def test_full_size_step_as_benched(index):
+    """BASELINE.json full sizes in exactly the launch configuration bench.py times: channels-last,
+    forward first, then the backward with RAF_REUSE_PREP on the same workspace (two launches per
+    step).  Forward: sampled rows against the oracle.  Backward: a 16-channel slice against the
+    oracle (channels are independent), plus properties that hold at any size (untouched pixels
+    exactly zero, every element finite) on all channels."""
+    wl = inputs.make_workload(index)
+    cfg = wl.cfg
+    tdt = T.TORCH_DTYPE[cfg.dtype]
+    PH, PW = cfg.out_size
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    feats, _ = T.device_feats(wl.feats, cfg.dtype, "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    out = T.empty_layout((K, C, PH, PW), tdt, "cl", fill=float("nan"))
+    go_t = torch.from_numpy(wl.grad_out).to(tdt)
+    gout = T.to_layout(go_t.cuda(), "cl")
+    grads = [T.empty_layout(s_, torch.float32, "cl", fill=float("nan")) for s_ in cfg.level_shapes]
+    ws = T.workspace(K, L, PH, PW, 2, B.RAF_REUSE_PREP)
+    B.roi_align_fpn_forward(feats, cfg.scales, rois, out, 2, True, cfg.finest_scale, ws)
+    B.roi_align_fpn_backward(grads, cfg.scales, gout, rois, 2, True, cfg.finest_scale, B.RAF_REUSE_PREP, ws)
+    torch.cuda.synchronize()
+    # forward, sampled rows
+    pick = np.sort(np.random.default_rng(100 + index).choice(K, 32, replace=False))
+    exact = [f.to(torch.float64).cpu().numpy() for f in feats]
+    ref = R.forward(exact, cfg.scales, wl.rois[pick], (PH, PW), 2, True, cfg.finest_scale)
+    T.assert_forward_close(out[torch.from_numpy(pick).cuda()].to(torch.float64).cpu().numpy(), ref, cfg.dtype)
+    del exact
+    # backward, channel slice
+    sl = slice(96, 112)
+    shapes = [(s_[0], 16, s_[2], s_[3]) for s_ in cfg.level_shapes]
+    gref, S = R.backward(shapes, cfg.scales, go_t[:, sl].to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
+                         cfg.finest_scale)
+    T.assert_backward_close([g[:, sl].to(torch.float64).cpu().numpy() for g in grads], gref, S)
+    masks = R.footprint(cfg.level_shapes, cfg.scales, wl.rois, (PH, PW), 2, True)
+    for g, m in zip(grads, masks):
+        assert bool(torch.isfinite(g).all())
+        untouched = torch.from_numpy(m == 0).cuda()[:, None].expand_as(g)
+        assert bool((g[untouched] == 0).all())
+
+
 def test_adjoint_identity_on_gpu():
     """<A x, g> = <x, A^T g> with both sides from the CUDA path (fp32): a property at full config-2
     size that needs no oracle."""

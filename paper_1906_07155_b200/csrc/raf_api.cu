@@ -204,7 +204,8 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
     int32_t* boff = reinterpret_cast<int32_t*>(base + w.boff);
     int4* bwin = reinterpret_cast<int4*>(base + w.bwin);
     PullTap* taps = reinterpret_cast<PullTap*>(base + w.taps);
-    if (!(flags & RAF_REUSE_PREP)) {   // else: written by roi_align_fpn_forward on the same arguments
+    if (!(flags & RAF_REUSE_PREP) || K == 0) {   // else: written by roi_align_fpn_forward on the same arguments
+                                                 // (the forward writes nothing when K == 0)
       rc = launch_pull_prep(p, a, bperm, boff, bwin, taps, st);
       if (rc) return rc;
     }

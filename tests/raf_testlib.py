@@ -28,7 +28,8 @@ def empty_layout(shape, dtype, layout: str, device="cuda", fill=None) -> torch.T
 
 
 def workspace(K, L, PH, PW, g, flags=0):
-    return torch.empty(B.roi_align_fpn_workspace_bytes(K, L, PH, PW, g, flags), dtype=torch.uint8, device="cuda")
+    """Workspace filled with a non-zero pattern: stale contents must never be trusted by the library."""
+    return torch.full((B.roi_align_fpn_workspace_bytes(K, L, PH, PW, g, flags),), 0x7B, dtype=torch.uint8, device="cuda")
 
 
 def device_feats(feats_np, dtype: str, layout: str):

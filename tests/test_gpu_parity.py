@@ -393,6 +393,11 @@ def test_k_zero_and_overwrite_zero_fill():
     grads, _ = T.gpu_backward(shapes, [0.25, 0.125], np.zeros((0, 8, 7, 7), np.float32),
                               np.zeros((0, 5), np.float32), 2, True, 56.0, "cl")
     assert all(np.all(g == 0) for g in grads)      # overwrite mode writes every element
+    # K == 0 with RAF_REUSE_PREP: the forward wrote nothing into the (garbage-filled) workspace; the
+    # backward must not trust it
+    grads, _ = T.gpu_backward(shapes, [0.25, 0.125], np.zeros((0, 8, 7, 7), np.float32),
+                              np.zeros((0, 5), np.float32), 2, True, 56.0, "cl", flags=B.RAF_REUSE_PREP)
+    assert all(np.all(g == 0) for g in grads)
 
 
 def test_host_entry_points_match_device_path():

@@ -114,8 +114,12 @@ __device__ __forceinline__ void fwd_dispatch_x(int nx, const T* rp0, const T* rp
 
 // Channels-last forward.  CTA = (RoI, chunk of 32 channel-vectors); warp = output bin row(s);
 // lanes = channel vectors (16 bytes each: a warp-wide load covers 512 contiguous bytes).
-template <typename T>
-__global__ void __launch_bounds__(32 * kFwdWarps, RAF_FWD_MINB)
+#ifndef RAF_FWD_MINB7
+#define RAF_FWD_MINB7 4
+#endif
+// kThreads = 224 (7 warps: 7-row outputs, the common case) or 256: the register budget follows the real block size.
+template <typename T, int kThreads>
+__global__ void __launch_bounds__(kThreads, kThreads == 224 ? RAF_FWD_MINB7 : RAF_FWD_MINB)
 fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
               int64_t os_w, int chunks, const PullPrepOut prep) {
   using V = Vec16<T>;
@@ -266,11 +270,18 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
       const size_t psmem = (size_t)(nw + 1) * ((size_t)lv.L * lv.n + 1) * sizeof(int);
       if (psmem > smem) smem = psmem;
     }
-    if (smem > 48 * 1024 &&
-        cudaFuncSetAttribute(fwd_cl_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-      return RAF_ERR_CUDA;
-    fwd_cl_kernel<T><<<(unsigned)((int64_t)a.K * chunks + po.nblocks), 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2],
-                                                                                               os[3], chunks, po);
+    const unsigned grid = (unsigned)((int64_t)a.K * chunks + po.nblocks);
+    if (nw == 7) {
+      if (smem > 48 * 1024 &&
+          cudaFuncSetAttribute(fwd_cl_kernel<T, 224>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return RAF_ERR_CUDA;
+      fwd_cl_kernel<T, 224><<<grid, 224, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, po);
+    } else {
+      if (smem > 48 * 1024 &&
+          cudaFuncSetAttribute(fwd_cl_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return RAF_ERR_CUDA;
+      fwd_cl_kernel<T, 256><<<grid, 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, po);
+    }
   } else {
     if (prep) {   // generic path: the prep tables still get written, by their own launch
       const int rc = launch_pull_prep(lv, a, prep->bperm, prep->boff, prep->bwin, prep->taps, stream);

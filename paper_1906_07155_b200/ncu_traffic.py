@@ -2,8 +2,8 @@
 from the committed `ncu --set full` summaries under profiles/ (bench.py's `roofline.traffic` field: it
 cannot be measured inside a timed run).  Keyed by BASELINE.json config index and bench leg."""
 
-# profiles/r1_v5.md: fwd_cl_kernel<float> (with the prep blocks) 121.9 + 34.1 MB; bwd_pull_kernel<float,true>
-# 56.5 + 131.6 MB.  Writes below the algorithmic bytes = output still dirty in L2 at kernel end.
+# profiles/r1_v6.md: fwd_cl_kernel<float,224> (with the prep blocks) 122.3 + 34.2 MB; bwd_pull_kernel<float,true>
+# 56.5 + 129.9 MB.  Writes below the algorithmic bytes = output still dirty in L2 at kernel end.
 TRAFFIC_BYTES = {
-    2: {"fwd": 155_990_016, "bwd": 188_186_368, "source": "profiles/r1_v5.md"},
+    2: {"fwd": 156_569_856, "bwd": 186_424_832, "source": "profiles/r1_v6.md"},
 }

@@ -68,6 +68,11 @@ enum {
                              with different arguments the result is undefined (but memory-safe only
                              if K and the level shapes match).                                       */
 };
+/* Forward flags (roi_align_fpn_forward_ex). */
+enum {
+  RAF_NO_PREP = 16        /* forward only (inference): do not write the backward's prep tables; the
+                             workspace is not touched and `ws` may be NULL                           */
+};
 /* With neither RAF_DETERMINISTIC nor RAF_ATOMIC the library picks the pull variant when eligible
  * and the atomic variant otherwise. */
 
@@ -98,6 +103,12 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
                           int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
                           void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,
                           void* stream);
+
+/* Forward with flags: 0 = roi_align_fpn_forward; RAF_NO_PREP = gather only. */
+int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                             int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
+                             void* out, const int64_t* out_strides, int flags, void* ws, size_t ws_bytes,
+                             void* stream);
 
 /* Backward: exact transpose of the forward.
  *   grad_feats   HOST array of L descriptors; data = fp32 DEVICE gradient pyramid, same logical

@@ -15,12 +15,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libraf.so")
 
 RAF_F32, RAF_F16, RAF_BF16 = 0, 1, 2
-RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC, RAF_REUSE_PREP = 1, 2, 4, 8
+RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC, RAF_REUSE_PREP, RAF_NO_PREP = 1, 2, 4, 8, 16
 _DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_BF16}
 
 EXPORTS = [
     "roi_align_fpn_workspace_bytes", "roi_fpn_assign_levels", "roi_align_fpn_forward",
-    "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
+    "roi_align_fpn_forward_ex", "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
 ]
 
@@ -68,6 +68,8 @@ def lib() -> ctypes.CDLL:
                            ("roi_align_fpn_backward", bwd_args), ("roi_align_fpn_backward_host", bwd_args)):
             getattr(L, name).restype = ctypes.c_int
             getattr(L, name).argtypes = args
+        L.roi_align_fpn_forward_ex.restype = ctypes.c_int
+        L.roi_align_fpn_forward_ex.argtypes = fwd_args[:12] + [ctypes.c_int] + fwd_args[12:]
         L.roi_align_fpn_strerror.restype = ctypes.c_char_p
         L.roi_align_fpn_strerror.argtypes = [ctypes.c_int]
         L.roi_align_fpn_launch_count.restype = ctypes.c_uint64
@@ -126,15 +128,66 @@ def roi_fpn_assign_levels(rois: torch.Tensor, L: int, finest_scale: float,
         raise RafError(rc, "roi_fpn_assign_levels")
 
 
+def _check_call(levels: Sequence[torch.Tensor], level_dtype, rois: torch.Tensor, roi_tensor: torch.Tensor,
+                roi_tensor_dtype, ws: Optional[torch.Tensor], host: bool = False) -> None:
+    """What the C ABI cannot see from raw pointers: dtypes, shapes, contiguity of `rois`, devices.
+    Raises ValueError before anything is passed down."""
+    if len(levels) == 0:
+        raise ValueError("no levels")
+    if rois.dtype != torch.float32 or rois.dim() != 2 or rois.shape[1] != 5 or not rois.is_contiguous():
+        raise ValueError("rois must be a contiguous float32 [K,5] tensor")
+    if roi_tensor.dim() != 4 or roi_tensor.shape[0] != rois.shape[0]:
+        raise ValueError("out / grad_out must be logical [K,C,PH,PW] with K = rois.shape[0]")
+    if roi_tensor.dtype != roi_tensor_dtype:
+        raise ValueError(f"out / grad_out dtype {roi_tensor.dtype} does not match {roi_tensor_dtype}")
+    for t in levels:
+        if t.dim() != 4 or t.dtype != level_dtype:
+            raise ValueError(f"every level must be a 4-d {level_dtype} tensor")
+        if t.shape[0] != levels[0].shape[0] or t.shape[1] != levels[0].shape[1]:
+            raise ValueError("N and C must be identical across levels")
+    if roi_tensor.shape[1] != levels[0].shape[1]:
+        raise ValueError("out / grad_out channel count differs from the levels'")
+    tensors = list(levels) + [rois, roi_tensor] + ([ws] if ws is not None and not host else [])
+    if host:
+        if any(t.is_cuda for t in tensors):
+            raise ValueError("the *_host entry points take host tensors")
+        if ws is None or not ws.is_cuda:
+            raise ValueError("arena must be a CUDA tensor")
+    else:
+        if not all(t.is_cuda for t in tensors) or len({t.device for t in tensors}) != 1:
+            raise ValueError("all tensors must live on the same CUDA device")
+
+
+def roi_align_fpn_forward_ex(feats: Sequence[torch.Tensor], scales: Sequence[float], rois: torch.Tensor,
+                             out: torch.Tensor, sampling_ratio: int, aligned: bool, finest_scale: float,
+                             flags: int, ws: Optional[torch.Tensor], stream=None, levels_desc=None) -> None:
+    """out: logical [K,C,PH,PW] tensor of any strides (e.g. a permuted view of a [K,PH,PW,C] buffer).
+    flags: 0 or RAF_NO_PREP (forward only: `ws` may be None)."""
+    _check_call(feats, feats[0].dtype if len(feats) else None, rois, out, feats[0].dtype if len(feats) else None, ws)
+    if feats[0].dtype not in _DTYPES:
+        raise ValueError(f"unsupported feature dtype {feats[0].dtype}")
+    desc = levels_desc if levels_desc is not None else make_levels(feats, scales)
+    K, _, PH, PW = out.shape
+    rc = lib().roi_align_fpn_forward_ex(desc, len(feats), _DTYPES[feats[0].dtype], _ptr(rois), K, PH, PW,
+                                        sampling_ratio, int(bool(aligned)), finest_scale, _ptr(out),
+                                        _strides4(out), int(flags), _ptr(ws),
+                                        0 if ws is None else ws.numel() * ws.element_size(), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fpn_forward_ex")
+
+
 def roi_align_fpn_forward(feats: Sequence[torch.Tensor], scales: Sequence[float], rois: torch.Tensor,
                           out: torch.Tensor, sampling_ratio: int, aligned: bool, finest_scale: float,
                           ws: torch.Tensor, stream=None, levels_desc=None) -> None:
     """out: logical [K,C,PH,PW] tensor of any strides (e.g. a permuted view of a [K,PH,PW,C] buffer)."""
+    _check_call(feats, feats[0].dtype if len(feats) else None, rois, out, feats[0].dtype if len(feats) else None, ws)
+    if feats[0].dtype not in _DTYPES:
+        raise ValueError(f"unsupported feature dtype {feats[0].dtype}")
     desc = levels_desc if levels_desc is not None else make_levels(feats, scales)
     K, _, PH, PW = out.shape
     rc = lib().roi_align_fpn_forward(desc, len(feats), _DTYPES[feats[0].dtype], _ptr(rois), K, PH, PW,
                                      sampling_ratio, int(bool(aligned)), finest_scale, _ptr(out),
-                                     _strides4(out), _ptr(ws), ws.numel() * ws.element_size(),
+                                     _strides4(out), _ptr(ws), 0 if ws is None else ws.numel() * ws.element_size(),
                                      _stream_ptr(stream))
     if rc:
         raise RafError(rc, "roi_align_fpn_forward")
@@ -144,6 +197,9 @@ def roi_align_fpn_backward(grad_feats: Sequence[torch.Tensor], scales: Sequence[
                            grad_out: torch.Tensor, rois: torch.Tensor, sampling_ratio: int,
                            aligned: bool, finest_scale: float, flags: int, ws: torch.Tensor,
                            stream=None, levels_desc=None) -> None:
+    if grad_out.dtype not in _DTYPES:
+        raise ValueError(f"unsupported grad_out dtype {grad_out.dtype}")
+    _check_call(grad_feats, torch.float32, rois, grad_out, grad_out.dtype, ws)
     desc = levels_desc if levels_desc is not None else make_levels(grad_feats, scales)
     K, _, PH, PW = grad_out.shape
     rc = lib().roi_align_fpn_backward(desc, len(grad_feats), _DTYPES[grad_out.dtype], _ptr(grad_out),
@@ -165,6 +221,8 @@ def roi_align_fpn_forward_host(feats_host: Sequence[torch.Tensor], scales, rois_
                                out_host: torch.Tensor, sampling_ratio: int, aligned: bool,
                                finest_scale: float, arena: torch.Tensor, stream=None) -> None:
     """HOST (pinned) tensors in and out; `arena` is a device byte buffer."""
+    _check_call(feats_host, feats_host[0].dtype if len(feats_host) else None, rois_host, out_host,
+                feats_host[0].dtype if len(feats_host) else None, arena, host=True)
     desc = make_levels(feats_host, scales)
     K, _, PH, PW = out_host.shape
     rc = lib().roi_align_fpn_forward_host(desc, len(feats_host), _DTYPES[feats_host[0].dtype],
@@ -179,6 +237,7 @@ def roi_align_fpn_backward_host(grad_feats_host: Sequence[torch.Tensor], scales,
                                 grad_out_host: torch.Tensor, rois_host: torch.Tensor,
                                 sampling_ratio: int, aligned: bool, finest_scale: float, flags: int,
                                 arena: torch.Tensor, stream=None) -> None:
+    _check_call(grad_feats_host, torch.float32, rois_host, grad_out_host, grad_out_host.dtype, arena, host=True)
     desc = make_levels(grad_feats_host, scales)
     K, _, PH, PW = grad_out_host.shape
     rc = lib().roi_align_fpn_backward_host(desc, len(grad_feats_host), _DTYPES[grad_out_host.dtype],

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libraf.so")
-SOURCES = ["raf_api.cu", "raf_levels.cu", "raf_forward.cu", "raf_forward_tma.cu", "raf_backward.cu",
+SOURCES = ["raf_api.cu", "raf_levels.cu", "raf_forward.cu", "raf_backward.cu",
            "raf_backward_pull.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--cudart", "shared"]
@@ -22,8 +22,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source_mtime():
         return LIB
     cmd = ["nvcc"] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
-    if os.environ.get("RAF_FWD_TMA") == "1":   # experimental: dispatch the bulk-async forward (raf_forward_tma.cu)
-        cmd.append("-DRAF_FWD_TMA")
+    cmd += os.environ.get("RAF_NVCC_EXTRA", "").split()   # e.g. -DRAF_EXPERIMENT (tuning knobs read from the environment)
     cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB + ".tmp"]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)

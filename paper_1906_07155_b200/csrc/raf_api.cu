@@ -88,39 +88,74 @@ using namespace raf;
 
 extern "C" {
 
-// Workspace carve-up (pull backward): [bperm K int32][boff kBoffInts int32][bwin K int4][taps].
+// Workspace carve-up (pull backward): [hdr 256 B][bperm K int32][boff kBoffInts int32][bwin K int4][inv].
 struct WsLayout {
-  size_t bperm, boff, bwin, taps, total;
+  size_t hdr, bperm, boff, bwin, inv, total;
 };
-static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
+static WsLayout ws_layout(int K) {
   const size_t k = K > 0 ? (size_t)K : 0;
-  const size_t g = sampling_ratio > 0 ? (size_t)sampling_ratio : 0;
   WsLayout w;
+  w.hdr = 0;
   w.bperm = 256;
   w.boff = w.bperm + align256(4 * k);
   w.bwin = w.boff + align256(4 * (size_t)kBoffInts);
-  w.taps = w.bwin + align256(16 * k);
-  w.total = w.taps + align256(k * (size_t)(out_h + out_w) * 2 * g * sizeof(PullTap)) + 256;
+  w.inv = w.bwin + align256(16 * k);
+  w.total = w.inv + align256(k * 2 * kInvCap * sizeof(InvEntry)) + 256;
   return w;
 }
 
 // The pull backward's prep tables can be built for these arguments (layout-independent part of the
 // pull eligibility; the forward uses the same test before it writes them into the workspace).
-static bool prep_possible(const raf_level* lv, int L, int sampling_ratio) {
-  if (sampling_ratio <= 0 || (int64_t)L * lv[0].n + 1 > kBoffInts) return false;
+static bool prep_possible(const raf_level* lv, int L) {
+  if ((int64_t)L * lv[0].n + 1 > kBoffInts) return false;
   if (bucket_smem_bytes(L, lv[0].n) > 200 * 1024) return false;
   if ((size_t)(kMaxLevels + 1) * ((size_t)L * lv[0].n + 1) * sizeof(int) > 200 * 1024) return false;
-  for (int l = 0; l < L; ++l)   // tap tables keep pixel indices in 24 bits
-    if (lv[l].h >= 0xffffff || lv[l].w >= 0xffffff) return false;
   return true;
+}
+
+// 64-bit FNV-1a over the arguments the prep tables depend on.
+static void fnv(uint64_t& h, const void* p, size_t n) {
+  const unsigned char* b = (const unsigned char*)p;
+  for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+}
+static PrepFingerprint prep_fingerprint(const raf_level* lv, int L, const float* rois, int K, int out_h, int out_w,
+                                        int sampling_ratio, int aligned, float finest_scale) {
+  uint64_t h = 1469598103934665603ull;
+  for (int l = 0; l < L; ++l) {
+    fnv(h, &lv[l].h, sizeof(int32_t)); fnv(h, &lv[l].w, sizeof(int32_t));
+    fnv(h, &lv[l].spatial_scale, sizeof(float));
+  }
+  PrepFingerprint f;
+  f.v[0] = 0x52414632u;   // "RAF2": table format
+  f.v[1] = (uint32_t)K;
+  f.v[2] = (uint32_t)out_h | ((uint32_t)out_w << 8) | ((uint32_t)sampling_ratio << 16) | ((uint32_t)(aligned ? 1 : 0) << 24) |
+           ((uint32_t)L << 25);
+  std::memcpy(&f.v[3], &finest_scale, 4);
+  f.v[4] = (uint32_t)lv[0].n;
+  f.v[5] = (uint32_t)(h ^ (h >> 32));
+  const uint64_t rp = (uint64_t)(uintptr_t)rois;
+  f.v[6] = (uint32_t)rp;
+  f.v[7] = (uint32_t)(rp >> 32);
+  return f;
+}
+
+static PullPrepOut prep_out(void* ws, int K, const PrepFingerprint& fp) {
+  const WsLayout w = ws_layout(K);
+  char* base = reinterpret_cast<char*>(ws);
+  PullPrepOut po{};
+  po.hdr = reinterpret_cast<uint32_t*>(base + w.hdr);
+  po.bperm = reinterpret_cast<int32_t*>(base + w.bperm);
+  po.boff = reinterpret_cast<int32_t*>(base + w.boff);
+  po.bwin = reinterpret_cast<int4*>(base + w.bwin);
+  po.inv = reinterpret_cast<InvEntry*>(base + w.inv);
+  po.fp = fp;
+  return po;
 }
 
 size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,
                                      int flags) {
-  (void)L; (void)flags;
-  if (out_h < 1) out_h = 1;
-  if (out_w < 1) out_w = 1;
-  return ws_layout(K, out_h, out_w, sampling_ratio).total;
+  (void)L; (void)flags; (void)out_h; (void)out_w; (void)sampling_ratio;
+  return ws_layout(K).total;
 }
 
 int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
@@ -137,6 +172,14 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
                           int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
                           void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,
                           void* stream) {
+  return roi_align_fpn_forward_ex(feats, L, dtype, rois, K, out_h, out_w, sampling_ratio, aligned, finest_scale,
+                                  out, out_strides, 0, ws, ws_bytes, stream);
+}
+
+int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                             int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
+                             void* out, const int64_t* out_strides, int flags, void* ws, size_t ws_bytes,
+                             void* stream) {
   int rc = check_levels(feats, L);
   if (rc) return rc;
   rc = check_common(rois, K, out_h, out_w, sampling_ratio);
@@ -147,8 +190,13 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
   if (K == 0) return RAF_OK;  // nothing to do; strides of an empty tensor are not meaningful
   for (int i = 0; i < 4; ++i) if (out_strides[i] <= 0) return RAF_ERR_STRIDE;
   if (!out) return RAF_ERR_NULL;
-  if (!ws) return RAF_ERR_NULL;
-  if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, 0)) return RAF_ERR_WORKSPACE;
+  if (flags & ~RAF_NO_PREP) return RAF_ERR_UNSUPPORTED;
+  const bool want_prep = !(flags & RAF_NO_PREP);
+  if (want_prep) {
+    if (!ws) return RAF_ERR_NULL;
+    if ((uintptr_t)ws % 256) return RAF_ERR_WORKSPACE;
+    if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, 0)) return RAF_ERR_WORKSPACE;
+  }
 
   LevelsParam p;
   fill_param(feats, L, &p);
@@ -157,16 +205,10 @@ int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const 
   const bool cl = levels_vectorizable(feats, L, vec, esize(dtype)) &&
                   tensor_vectorizable(out, out_strides, vec, esize(dtype));
   // the workspace receives the pull backward's prep tables (consumed by RAF_REUSE_PREP)
-  PullPrepOut po{nullptr, nullptr, nullptr, nullptr, 0};
-  const bool with_prep = prep_possible(feats, L, sampling_ratio);
-  if (with_prep) {
-    const WsLayout w = ws_layout(K, out_h, out_w, sampling_ratio);
-    char* base = reinterpret_cast<char*>(ws);
-    po.bperm = reinterpret_cast<int32_t*>(base + w.bperm);
-    po.boff = reinterpret_cast<int32_t*>(base + w.boff);
-    po.bwin = reinterpret_cast<int4*>(base + w.bwin);
-    po.taps = reinterpret_cast<PullTap*>(base + w.taps);
-  }
+  PullPrepOut po{};
+  const bool with_prep = want_prep && prep_possible(feats, L);
+  if (with_prep)
+    po = prep_out(ws, K, prep_fingerprint(feats, L, rois, K, out_h, out_w, sampling_ratio, aligned, finest_scale));
   return launch_forward(p, dtype, a, out, out_strides, cl, with_prep ? &po : nullptr, (cudaStream_t)stream);
 }
 
@@ -186,6 +228,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
   if (K > 0 && !grad_out) return RAF_ERR_NULL;
   if (!ws) return RAF_ERR_NULL;
+  if ((uintptr_t)ws % 256) return RAF_ERR_WORKSPACE;
   if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
     return RAF_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
@@ -196,21 +239,19 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                   (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype)));
 
   // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
-  const bool pull_ok = cl && prep_possible(grad_feats, L, sampling_ratio);
+  const bool pull_ok = cl && prep_possible(grad_feats, L);
   if (pull_ok && !(flags & RAF_ATOMIC)) {
-    const WsLayout w = ws_layout(K, out_h, out_w, sampling_ratio);
-    char* base = reinterpret_cast<char*>(ws);
-    int32_t* bperm = reinterpret_cast<int32_t*>(base + w.bperm);
-    int32_t* boff = reinterpret_cast<int32_t*>(base + w.boff);
-    int4* bwin = reinterpret_cast<int4*>(base + w.bwin);
-    PullTap* taps = reinterpret_cast<PullTap*>(base + w.taps);
-    if (!(flags & RAF_REUSE_PREP) || K == 0) {   // else: written by roi_align_fpn_forward on the same arguments
-                                                 // (the forward writes nothing when K == 0)
-      rc = launch_pull_prep(p, a, bperm, boff, bwin, taps, st);
-      if (rc) return rc;
+    const PullPrepOut po = prep_out(ws, K, prep_fingerprint(grad_feats, L, rois, K, out_h, out_w, sampling_ratio, aligned,
+                                                           finest_scale));
+    rc = pull_eligible(p, gout_dtype, a, grad_out, gout_strides);
+    if (rc == RAF_OK) {
+      if (!(flags & RAF_REUSE_PREP) || K == 0) {   // else: written by roi_align_fpn_forward on the same arguments
+                                                   // (the forward writes nothing when K == 0); the kernel checks
+        rc = launch_pull_prep(p, a, po, st);
+        if (rc) return rc;
+      }
+      return launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, po, (flags & RAF_ACCUMULATE) ? 1 : 0, st);
     }
-    rc = launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, bperm, boff, bwin, taps,
-                              (flags & RAF_ACCUMULATE) ? 1 : 0, st);
     if (rc != RAF_ERR_UNSUPPORTED) return rc;
   }
   if (flags & RAF_DETERMINISTIC) return RAF_ERR_UNSUPPORTED;

@@ -131,11 +131,15 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   int* s_cnt = reinterpret_cast<int*>(s_tab + nb * slots);     // [PH + PW]
   __shared__ int s_b;
 
-  if ((int)blockIdx.x < prep.nblocks) {   // leading blocks: the backward's prep tables (same RoIs, same
-    pull_prep_block(lv, a, prep, (int)blockIdx.x, reinterpret_cast<int*>(fwd_smem));   // geometry), for free
+  // The backward's prep rides in this launch (same RoIs, same geometry): block 0 buckets the RoIs (a
+  // serial chain, so it starts first), the blocks after the forward's own write the inverse tap tables
+  // (independent items: they fill the tail of the grid).
+  const int nfwd = a.K * chunks;
+  if (prep.nblocks > 0 && ((int)blockIdx.x == 0 || (int)blockIdx.x > nfwd)) {
+    pull_prep_block(lv, a, prep, (int)blockIdx.x == 0 ? 0 : (int)blockIdx.x - nfwd, reinterpret_cast<int*>(fwd_smem));
     return;
   }
-  const int bid = (int)blockIdx.x - prep.nblocks;
+  const int bid = (int)blockIdx.x - (prep.nblocks > 0 ? 1 : 0);
   const int k = bid / chunks, chunk = bid - k * chunks;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   const float* r = a.rois + 5 * (int64_t)k;
@@ -263,8 +267,8 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
     size_t smem = (size_t)(a.PH + a.PW) * (2 * g * sizeof(FwdTap) + sizeof(int));
     int nw = a.PH < kFwdWarps ? a.PH : kFwdWarps;          // one warp per output bin row
     while (32 * nw < a.PH + a.PW) ++nw;                     // the table set-up needs PH + PW threads
-    PullPrepOut po{nullptr, nullptr, nullptr, nullptr, 0};
-    if (prep) {                                             // carry the backward's prep in the leading blocks
+    PullPrepOut po{};
+    if (prep) {                                             // carry the backward's prep in extra blocks
       po = *prep;
       po.nblocks = pull_prep_blocks(a, 32 * nw);
       const size_t psmem = (size_t)(nw + 1) * ((size_t)lv.L * lv.n + 1) * sizeof(int);
@@ -284,7 +288,7 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
     }
   } else {
     if (prep) {   // generic path: the prep tables still get written, by their own launch
-      const int rc = launch_pull_prep(lv, a, prep->bperm, prep->boff, prep->bwin, prep->taps, stream);
+      const int rc = launch_pull_prep(lv, a, *prep, stream);
       if (rc) return rc;
     }
     const int64_t total = (int64_t)a.K * lv.c * a.PH * a.PW;
@@ -298,15 +302,6 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
 
 int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
                    const int64_t* out_strides, bool channels_last, const PullPrepOut* prep, cudaStream_t stream) {
-#ifdef RAF_FWD_TMA
-  if (channels_last) {   // bulk-async staged variant (raf_forward_tma.cu) where it applies
-    int rc = launch_forward_tma(lv, dtype, a, out, out_strides, stream);
-    if (rc != RAF_ERR_UNSUPPORTED) {
-      if (rc == RAF_OK && prep) rc = launch_pull_prep(lv, a, prep->bperm, prep->boff, prep->bwin, prep->taps, stream);
-      return rc;
-    }
-  }
-#endif
   switch (dtype) {
     case RAF_F32: return forward_typed<float>(lv, a, out, out_strides, channels_last, prep, stream);
     case RAF_F16: return forward_typed<__half>(lv, a, out, out_strides, channels_last, prep, stream);

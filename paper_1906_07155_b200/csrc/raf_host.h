@@ -32,33 +32,25 @@ struct PullPrepOut;
 int launch_forward(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
                    const int64_t* out_strides, bool channels_last, const PullPrepOut* prep, cudaStream_t stream);
 
-// Forward, bulk-async (TMA) staged variant; RAF_ERR_UNSUPPORTED when the arguments are outside its range.
-int launch_forward_tma(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, void* out,
-                       const int64_t* out_strides, cudaStream_t stream);
-
 // Backward (atomic scatter).  The gradient pyramid must already hold its starting values.
 int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a,
                            const void* grad_out, const int64_t* gout_strides, bool channels_last,
                            cudaStream_t stream);
 
-// One merged bilinear tap of an output bin along one axis (pull backward tap tables).
-struct PullTap {
-  uint32_t pb;  // pixel | bin << 24; pixel == 0xffffff marks an empty slot
-  float w;      // weight (y taps carry 1/count)
-};
-
-// Prep launch of the pull backward (sampling_ratio > 0): block 0 buckets the RoIs by (level, image)
-// -- bperm[K], boff[L*N + 1], bwin[K] = conservative touched-pixel window of every kept RoI in
-// bperm order -- and the other blocks write the tap tables taps[K][PH + PW][2 * sampling_ratio].
+// Prep launch of the pull backward: block 0 buckets the RoIs by (level, image) -- bperm[K],
+// boff[L*N + 1], bwin[K] = conservative touched-pixel window of every kept RoI in bperm order -- and
+// the other blocks write the inverse tap tables inv[K][2][kInvCap] (raf_pull_prep.cuh).
 size_t bucket_smem_bytes(int L, int N);
-int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, int32_t* bperm, int32_t* boff, int4* bwin,
-                     PullTap* taps, cudaStream_t stream);
+int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, const PullPrepOut& prep, cudaStream_t stream);
 
-// Backward, deterministic pull formulation (channels-last, sampling_ratio > 0).  Writes every
-// gradient element exactly once (or adds into it when `accumulate`).
+// Backward, deterministic pull formulation (channels-last).  Writes every gradient element exactly
+// once (or adds into it when `accumulate`).  `prep` = the tables launch_pull_prep (or the forward) left
+// in the workspace for the same arguments, with the fingerprint the kernel checks them against.
+// RAF_OK when launch_backward_pull takes these arguments, RAF_ERR_UNSUPPORTED otherwise (host-side test).
+int pull_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
+                  const int64_t* gout_strides);
 int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
-                         const int64_t* gout_strides, const int32_t* bperm, const int32_t* boff,
-                         const int4* bwin, const PullTap* taps, int accumulate, cudaStream_t stream);
+                         const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream);
 
 // Zero-fill of one strided level (used when the level is not one dense block).
 int launch_zero_level(float* data, int n, int c, int h, int w, int64_t sn, int64_t sc, int64_t sh,

@@ -88,28 +88,31 @@ using namespace raf;
 
 extern "C" {
 
-// Workspace carve-up (pull backward): [hdr 256 B][bperm K int32][boff kBoffInts int32][bwin K int4][inv].
+// Workspace carve-up (pull backward): [hdr 256 B][bperm K int32][boff kBoffInts int32][bwin K int4][taps].
 struct WsLayout {
-  size_t hdr, bperm, boff, bwin, inv, total;
+  size_t hdr, bperm, boff, bwin, taps, total;
 };
-static WsLayout ws_layout(int K) {
+static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
   const size_t k = K > 0 ? (size_t)K : 0;
+  const size_t g = sampling_ratio > 0 ? (size_t)sampling_ratio : 0;
   WsLayout w;
   w.hdr = 0;
   w.bperm = 256;
   w.boff = w.bperm + align256(4 * k);
   w.bwin = w.boff + align256(4 * (size_t)kBoffInts);
-  w.inv = w.bwin + align256(16 * k);
-  w.total = w.inv + align256(k * 2 * kInvCap * sizeof(InvEntry)) + 256;
+  w.taps = w.bwin + align256(16 * k);
+  w.total = w.taps + align256(k * (size_t)(out_h + out_w) * 2 * g * sizeof(PullTap)) + 256;
   return w;
 }
 
 // The pull backward's prep tables can be built for these arguments (layout-independent part of the
 // pull eligibility; the forward uses the same test before it writes them into the workspace).
-static bool prep_possible(const raf_level* lv, int L) {
-  if ((int64_t)L * lv[0].n + 1 > kBoffInts) return false;
+static bool prep_possible(const raf_level* lv, int L, int sampling_ratio) {
+  if (sampling_ratio <= 0 || (int64_t)L * lv[0].n + 1 > kBoffInts) return false;
   if (bucket_smem_bytes(L, lv[0].n) > 200 * 1024) return false;
   if ((size_t)(kMaxLevels + 1) * ((size_t)L * lv[0].n + 1) * sizeof(int) > 200 * 1024) return false;
+  for (int l = 0; l < L; ++l)   // tap tables keep pixel indices in 24 bits
+    if (lv[l].h >= 0xffffff || lv[l].w >= 0xffffff) return false;
   return true;
 }
 
@@ -126,7 +129,7 @@ static PrepFingerprint prep_fingerprint(const raf_level* lv, int L, const float*
     fnv(h, &lv[l].spatial_scale, sizeof(float));
   }
   PrepFingerprint f;
-  f.v[0] = 0x52414632u;   // "RAF2": table format
+  f.v[0] = 0x52414631u;   // "RAF1": table format
   f.v[1] = (uint32_t)K;
   f.v[2] = (uint32_t)out_h | ((uint32_t)out_w << 8) | ((uint32_t)sampling_ratio << 16) | ((uint32_t)(aligned ? 1 : 0) << 24) |
            ((uint32_t)L << 25);
@@ -139,23 +142,25 @@ static PrepFingerprint prep_fingerprint(const raf_level* lv, int L, const float*
   return f;
 }
 
-static PullPrepOut prep_out(void* ws, int K, const PrepFingerprint& fp) {
-  const WsLayout w = ws_layout(K);
+static PullPrepOut prep_out(void* ws, int K, int out_h, int out_w, int sampling_ratio, const PrepFingerprint& fp) {
+  const WsLayout w = ws_layout(K, out_h, out_w, sampling_ratio);
   char* base = reinterpret_cast<char*>(ws);
   PullPrepOut po{};
   po.hdr = reinterpret_cast<uint32_t*>(base + w.hdr);
   po.bperm = reinterpret_cast<int32_t*>(base + w.bperm);
   po.boff = reinterpret_cast<int32_t*>(base + w.boff);
   po.bwin = reinterpret_cast<int4*>(base + w.bwin);
-  po.inv = reinterpret_cast<InvEntry*>(base + w.inv);
+  po.taps = reinterpret_cast<PullTap*>(base + w.taps);
   po.fp = fp;
   return po;
 }
 
 size_t roi_align_fpn_workspace_bytes(int K, int L, int out_h, int out_w, int sampling_ratio,
                                      int flags) {
-  (void)L; (void)flags; (void)out_h; (void)out_w; (void)sampling_ratio;
-  return ws_layout(K).total;
+  (void)L; (void)flags;
+  if (out_h < 1) out_h = 1;
+  if (out_w < 1) out_w = 1;
+  return ws_layout(K, out_h, out_w, sampling_ratio).total;
 }
 
 int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, int32_t* levels,
@@ -206,9 +211,9 @@ int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, con
                   tensor_vectorizable(out, out_strides, vec, esize(dtype));
   // the workspace receives the pull backward's prep tables (consumed by RAF_REUSE_PREP)
   PullPrepOut po{};
-  const bool with_prep = want_prep && prep_possible(feats, L);
+  const bool with_prep = want_prep && prep_possible(feats, L, sampling_ratio);
   if (with_prep)
-    po = prep_out(ws, K, prep_fingerprint(feats, L, rois, K, out_h, out_w, sampling_ratio, aligned, finest_scale));
+    po = prep_out(ws, K, out_h, out_w, sampling_ratio, prep_fingerprint(feats, L, rois, K, out_h, out_w, sampling_ratio, aligned, finest_scale));
   return launch_forward(p, dtype, a, out, out_strides, cl, with_prep ? &po : nullptr, (cudaStream_t)stream);
 }
 
@@ -239,9 +244,9 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                   (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype)));
 
   // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
-  const bool pull_ok = cl && prep_possible(grad_feats, L);
+  const bool pull_ok = cl && prep_possible(grad_feats, L, sampling_ratio);
   if (pull_ok && !(flags & RAF_ATOMIC)) {
-    const PullPrepOut po = prep_out(ws, K, prep_fingerprint(grad_feats, L, rois, K, out_h, out_w, sampling_ratio, aligned,
+    const PullPrepOut po = prep_out(ws, K, out_h, out_w, sampling_ratio, prep_fingerprint(grad_feats, L, rois, K, out_h, out_w, sampling_ratio, aligned,
                                                            finest_scale));
     rc = pull_eligible(p, gout_dtype, a, grad_out, gout_strides);
     if (rc == RAF_OK) {

@@ -132,7 +132,7 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   __shared__ int s_b;
 
   // The backward's prep rides in this launch (same RoIs, same geometry): block 0 buckets the RoIs (a
-  // serial chain, so it starts first), the blocks after the forward's own write the inverse tap tables
+  // serial chain, so it starts first), the blocks after the forward's own write the tap tables
   // (independent items: they fill the tail of the grid).
   const int nfwd = a.K * chunks;
   if (prep.nblocks > 0 && ((int)blockIdx.x == 0 || (int)blockIdx.x > nfwd)) {

@@ -37,18 +37,26 @@ int launch_backward_atomic(const LevelsParam& glv, raf_dtype gout_dtype, const R
                            const void* grad_out, const int64_t* gout_strides, bool channels_last,
                            cudaStream_t stream);
 
-// Prep launch of the pull backward: block 0 buckets the RoIs by (level, image) -- bperm[K],
-// boff[L*N + 1], bwin[K] = conservative touched-pixel window of every kept RoI in bperm order -- and
-// the other blocks write the inverse tap tables inv[K][2][kInvCap] (raf_pull_prep.cuh).
+// One merged bilinear tap of an output bin along one axis (pull backward tap tables).
+struct PullTap {
+  uint32_t pb;  // pixel | bin << 24; pixel == 0xffffff marks an empty slot
+  float w;      // weight (y taps carry 1/count)
+};
+
+// Prep launch of the pull backward (sampling_ratio > 0): block 0 buckets the RoIs by (level, image)
+// -- bperm[K], boff[L*N + 1], bwin[K] = conservative touched-pixel window of every kept RoI in
+// bperm order -- and writes the argument fingerprint; the other blocks write the tap tables
+// taps[K][PH + PW][2 * sampling_ratio] (raf_pull_prep.cuh).
 size_t bucket_smem_bytes(int L, int N);
 int launch_pull_prep(const LevelsParam& lv, const RoiArgs& a, const PullPrepOut& prep, cudaStream_t stream);
 
-// Backward, deterministic pull formulation (channels-last).  Writes every gradient element exactly
-// once (or adds into it when `accumulate`).  `prep` = the tables launch_pull_prep (or the forward) left
-// in the workspace for the same arguments, with the fingerprint the kernel checks them against.
 // RAF_OK when launch_backward_pull takes these arguments, RAF_ERR_UNSUPPORTED otherwise (host-side test).
 int pull_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
                   const int64_t* gout_strides);
+// Backward, deterministic pull formulation (channels-last, sampling_ratio > 0).  Writes every
+// gradient element exactly once (or adds into it when `accumulate`).  `prep` = the tables
+// launch_pull_prep (or the forward) left in the workspace for the same arguments, with the
+// fingerprint the kernel checks them against.
 int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
                          const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream);
 

@@ -16,6 +16,7 @@
 #include "raf_device.cuh"
 #include "raf_host.h"
 #include "raf_pull_prep.cuh"
+#include <cstdlib>
 
 namespace raf {
 
@@ -118,10 +119,11 @@ __device__ __forceinline__ void fwd_dispatch_x(int nx, const T* rp0, const T* rp
 #define RAF_FWD_MINB7 4
 #endif
 // kThreads = 224 (7 warps: 7-row outputs, the common case) or 256: the register budget follows the real block size.
+// A RoI's bin rows are split over `rsplit` CTAs (rows_per rows each) when there are more rows than warps.
 template <typename T, int kThreads>
-__global__ void __launch_bounds__(kThreads, kThreads == 224 ? RAF_FWD_MINB7 : RAF_FWD_MINB)
+__global__ void __launch_bounds__(kThreads, kThreads == 224 ? RAF_FWD_MINB7 : (kThreads == 128 ? 7 : RAF_FWD_MINB))
 fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
-              int64_t os_w, int chunks, const PullPrepOut prep) {
+              int64_t os_w, int chunks, int rsplit, int rows_per, const PullPrepOut prep) {
   using V = Vec16<T>;
   constexpr int VN = V::N;
   extern __shared__ __align__(16) unsigned char fwd_smem[];
@@ -134,13 +136,15 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   // The backward's prep rides in this launch (same RoIs, same geometry): block 0 buckets the RoIs (a
   // serial chain, so it starts first), the blocks after the forward's own write the tap tables
   // (independent items: they fill the tail of the grid).
-  const int nfwd = a.K * chunks;
+  const int nfwd = a.K * chunks * rsplit;
   if (prep.nblocks > 0 && ((int)blockIdx.x == 0 || (int)blockIdx.x > nfwd)) {
     pull_prep_block(lv, a, prep, (int)blockIdx.x == 0 ? 0 : (int)blockIdx.x - nfwd, reinterpret_cast<int*>(fwd_smem));
     return;
   }
   const int bid = (int)blockIdx.x - (prep.nblocks > 0 ? 1 : 0);
-  const int k = bid / chunks, chunk = bid - k * chunks;
+  const int part = bid % rsplit, kc = bid / rsplit;
+  const int k = kc / chunks, chunk = kc - k * chunks;
+  const int rbeg = part * rows_per, rend = min(PH, rbeg + rows_per);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
   const float* r = a.rois + 5 * (int64_t)k;
   const float r0 = __ldg(r), x1 = __ldg(r + 1), y1 = __ldg(r + 2), x2 = __ldg(r + 3), y2 = __ldg(r + 4);
@@ -162,7 +166,7 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   T* out_k = out + (int64_t)k * os_k + cv * VN;
   const T* base = reinterpret_cast<const T*>(lv.data[level]) + (int64_t)(b >= 0 ? b : 0) * lv.sn[level] + cv * VN;
 
-  for (int ph = warp; ph < PH; ph += nwarps) {
+  for (int ph = rbeg + warp; ph < rend; ph += nwarps) {
     const int ny = (b >= 0) ? s_cnt[ph] : 0;
     const FwdTap* ty = s_tab + ph * slots;
     float yw[4];
@@ -265,7 +269,15 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
     const int CV = lv.c / Vec16<T>::N;
     const int chunks = (CV + 31) / 32;
     size_t smem = (size_t)(a.PH + a.PW) * (2 * g * sizeof(FwdTap) + sizeof(int));
-    int nw = a.PH < kFwdWarps ? a.PH : kFwdWarps;          // one warp per output bin row
+    // one warp per bin row: outputs taller than 8 rows are split over several CTAs of equal height
+    // (14 rows: 2 x 7 warps -- measured 33.7 us vs 43.4 us for one CTA of 8 warps on config 4; splitting
+    // 7-row outputs into 4 + 3 rows is slower: 43.4 us vs 39.6 us on config 3)
+    int rsplit = (a.PH + kFwdWarps - 1) / kFwdWarps;
+#ifdef RAF_EXPERIMENT
+    if (const char* e = getenv("RAF_TUNE_RSPLIT")) rsplit = atoi(e);
+#endif
+    const int rows_per = (a.PH + rsplit - 1) / rsplit;
+    int nw = rows_per < kFwdWarps ? rows_per : kFwdWarps;   // one warp per output bin row
     while (32 * nw < a.PH + a.PW) ++nw;                     // the table set-up needs PH + PW threads
     PullPrepOut po{};
     if (prep) {                                             // carry the backward's prep in extra blocks
@@ -274,17 +286,22 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
       const size_t psmem = (size_t)(nw + 1) * ((size_t)lv.L * lv.n + 1) * sizeof(int);
       if (psmem > smem) smem = psmem;
     }
-    const unsigned grid = (unsigned)((int64_t)a.K * chunks + po.nblocks);
+    const unsigned grid = (unsigned)((int64_t)a.K * chunks * rsplit + po.nblocks);
     if (nw == 7) {
       if (smem > 48 * 1024 &&
           cudaFuncSetAttribute(fwd_cl_kernel<T, 224>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return RAF_ERR_CUDA;
-      fwd_cl_kernel<T, 224><<<grid, 224, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, po);
+      fwd_cl_kernel<T, 224><<<grid, 224, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, rsplit, rows_per, po);
+    } else if (nw <= 4) {
+      if (smem > 48 * 1024 &&
+          cudaFuncSetAttribute(fwd_cl_kernel<T, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return RAF_ERR_CUDA;
+      fwd_cl_kernel<T, 128><<<grid, 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, rsplit, rows_per, po);
     } else {
       if (smem > 48 * 1024 &&
           cudaFuncSetAttribute(fwd_cl_kernel<T, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return RAF_ERR_CUDA;
-      fwd_cl_kernel<T, 256><<<grid, 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, po);
+      fwd_cl_kernel<T, 256><<<grid, 32 * nw, smem, stream>>>(lv, a, o, os[0], os[2], os[3], chunks, rsplit, rows_per, po);
     }
   } else {
     if (prep) {   // generic path: the prep tables still get written, by their own launch

@@ -45,6 +45,10 @@ def parse_args():
     ap.add_argument("--rotate", type=int, default=0,
                     help="number of independent input/output buffer sets to rotate over (0 = cold-L2 protocol: "
                          "at least 4 and >= 2x L2; 1 = WARM single-buffer number, not the headline)")
+    ap.add_argument("--windows", type=int, default=5, help="timing windows per loop (median and min are reported)")
+    ap.add_argument("--window-iters", type=int, default=200, help="back-to-back iterations per timing window")
+    ap.add_argument("--sampling-ratio", type=int, default=None, help="override the config's sampling_ratio (0 = adaptive)")
+    ap.add_argument("--aligned", type=int, default=None, help="override the config's aligned flag (0 / 1)")
     ap.add_argument("--no-reuse-prep", action="store_true",
                     help="backward rebuilds its RoI buckets / tap tables instead of reusing the forward's (RAF_REUSE_PREP)")
     return ap.parse_args()
@@ -73,7 +77,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "25",
                  "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -153,11 +157,27 @@ class OracleLeg:
                           f"{t:.2f} s per pass"}
 
 
-def cpu_baseline(cfg_index, budget_s=20.0):
+def cpu_baseline(cfg_index, budget_s=14.0):
+    """The oracle on the host cores: all cores (OpenMP) on a bounded sample, then ONE thread on a smaller
+    sample (both sized from a probe so that the two legs together take about 20-25 s)."""
     leg = OracleLeg(cfg_index)
     leg.calibrate(budget_s)
     t = min(leg.run() for _ in range(3 if budget_s < 5 else 1))
-    return leg.describe(t, len(leg.sel) / t)
+    d = leg.describe(t, len(leg.sel) / t)
+    d["cpu_model"] = cpu_model()
+    try:   # the oracle is not touched: the OpenMP runtime it links is told to use one thread
+        import ctypes
+        gomp = ctypes.CDLL("libgomp.so.1")
+        cores = leg.R.num_threads()
+        gomp.omp_set_num_threads(1)
+        leg.calibrate(8.0)
+        t1 = leg.run()
+        d["single_thread"] = {"value": len(leg.sel) / t1, "unit": UNIT, "cores": leg.R.num_threads(),
+                              "sample": f"first {len(leg.sel) // leg.cfg.n_img} RoIs of each image, {t1:.2f} s per pass"}
+        gomp.omp_set_num_threads(cores)
+    except Exception as e:
+        d["single_thread"] = {"unavailable": str(e)}
+    return d
 
 
 def run_reference(args):
@@ -187,12 +207,47 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def source_hash():
+    """sha256 over the CUDA sources and the ABI header: identifies the build a profile was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1906_07155_b200", "csrc")
+    for f in sorted(os.listdir(csrc)) + [os.path.join("..", "..", "include", "raf.h")]:
+        with open(os.path.join(csrc, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config, variant):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) from profiles/traffic.json, which
+    bench_traffic.py writes from an `ncu --set full` report.  Only returned when it was measured on THIS build."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        t = json.load(open(p))
+    except Exception:
+        return {}, True
+    stale = t.get("source_hash") != source_hash()
+    entry = t.get("configs", {}).get(f"{config}:{variant}", {})
+    return ({} if stale else entry), stale
+
+
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
+    import bench_roofline as roofline
     from paper_1906_07155_b200 import binding as B
     from paper_1906_07155_b200 import build as raf_build
-    from paper_1906_07155_b200 import inputs, roofline
+    from paper_1906_07155_b200 import inputs
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -214,10 +269,16 @@ def run_ours(args):
     K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
     PH, PW = cfg.out_size
     g, aligned, fs = cfg.sampling_ratio, cfg.aligned, cfg.finest_scale
+    if args.sampling_ratio is not None:
+        g = args.sampling_ratio
+    if args.aligned is not None:
+        aligned = bool(args.aligned)
     flags = {"auto": 0, "atomic": B.RAF_ATOMIC, "deterministic": B.RAF_DETERMINISTIC}[args.backward]
-    if not args.no_reuse_prep and args.backward != "atomic":
+    reuse = cfg.backward and not args.no_reuse_prep and args.backward != "atomic" and g > 0
+    if reuse:
         flags |= B.RAF_REUSE_PREP   # a step runs the forward first, on the same RoIs and workspace: its launch
                                     # already wrote the backward's RoI buckets / tap tables (include/raf.h)
+    fwd_flags = 0 if cfg.backward else B.RAF_NO_PREP   # forward-only workloads do not build the backward's tables
 
     def lay(t):   # logical NCHW tensor -> requested physical layout
         return t.contiguous() if args.layout == "nchw" else t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
@@ -238,74 +299,87 @@ def run_ours(args):
     gdesc = [B.make_levels(gr, cfg.scales) for gr in grads] if cfg.backward else None
     stream = torch.cuda.current_stream()
 
-    def fwd(j):
-        B.roi_align_fpn_forward(feats[j], cfg.scales, rois, outs[j], g, aligned, fs, ws, stream, fdesc[j])
+    def fwd(j, s=stream):
+        B.roi_align_fpn_forward_ex(feats[j], cfg.scales, rois, outs[j], g, aligned, fs, fwd_flags, ws, s, fdesc[j])
 
-    def bwd(j):
-        B.roi_align_fpn_backward(grads[j], cfg.scales, gouts[j], rois, g, aligned, fs, flags, ws, stream, gdesc[j])
+    def bwd(j, s=stream):
+        B.roi_align_fpn_backward(grads[j], cfg.scales, gouts[j], rois, g, aligned, fs, flags, ws, s, gdesc[j])
+
+    def step(j, s=stream):
+        fwd(j, s)
+        if cfg.backward:
+            bwd(j, s)
 
     graphs = None
     if args.graph:
         graphs = []
         for j in range(R):
-            fwd(j)
-            if cfg.backward:
-                bwd(j)
+            step(j)
         torch.cuda.synchronize()
         for j in range(R):
             gr = torch.cuda.CUDAGraph()
             with torch.cuda.graph(gr):
-                s = torch.cuda.current_stream()
-                B.roi_align_fpn_forward(feats[j], cfg.scales, rois, outs[j], g, aligned, fs, ws, s, fdesc[j])
-                if cfg.backward:
-                    B.roi_align_fpn_backward(grads[j], cfg.scales, gouts[j], rois, g, aligned, fs, flags, ws, s, gdesc[j])
+                step(j, torch.cuda.current_stream())
             graphs.append(gr)
 
-    for i in range(args.warmup):
-        j = i % R
+    def run_step(j):
         if graphs:
             graphs[j].replay()
         else:
-            fwd(j)
-            if cfg.backward:
-                bwd(j)
+            step(j)
+
+    for i in range(args.warmup):
+        run_step(i % R)
     torch.cuda.synchronize()
 
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-        time.sleep(0.15)
+        time.sleep(0.1)
+
+    # ---- headline: EXACTLY `steps` interleaved fwd -> bwd steps between two events ----------------------
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     launches0 = B.launch_count()
+    e0.record(stream)
     for i in range(args.steps):
-        j = (args.warmup + i) % R
-        ev[i][0].record(stream)
-        if graphs:
-            graphs[j].replay()
-            ev[i][1].record(stream)
-        else:
-            fwd(j)
-            ev[i][1].record(stream)
-            if cfg.backward:
-                bwd(j)
-        ev[i][2].record(stream)
+        run_step((args.warmup + i) % R)
+    e1.record(stream)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     launches = B.launch_count() - launches0
+    per_step_launches = 1 + ((1 + L) if args.backward == "atomic" else (1 if reuse else 2)) * cfg.backward
     if graphs:   # replayed launches are not seen by the library's counter: count per captured step
-        launches = args.steps * (1 + ((1 + L) if args.backward == "atomic" else (1 if flags & B.RAF_REUSE_PREP else 2)) * cfg.backward)
-    total_ms = ev[0][0].elapsed_time(ev[-1][2])
+        launches = args.steps * per_step_launches
+    total_ms = e0.elapsed_time(e1)
     if world > 1:
         t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms = float(t.item())
+
+    # ---- SURVEY 8(d) protocol: windows of back-to-back iterations, median of >= 5 windows + min, for the
+    #      interleaved loop and for the forward-only / backward-only loops (the split) ---------------------
+    def windows(fn, n_windows=args.windows, iters=args.window_iters):
+        ms = []
+        for w in range(n_windows):
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(stream)
+            for i in range(iters):
+                fn((w * iters + i) % R)
+            a1.record(stream)
+            a1.synchronize()
+            ms.append(a0.elapsed_time(a1) / iters)
+        return {"median_ms": float(np.median(ms)), "min_ms": float(np.min(ms)), "windows": n_windows, "iters": iters}
+
+    loops = {"step": windows(run_step), "fwd": windows(fwd)}
+    if cfg.backward:
+        if reuse:   # the backward-only loop reuses the tables the last forward left in the workspace
+            fwd(0)
+        loops["bwd"] = windows(bwd)
     clocks = sampler.stop() if rank == 0 else None
-    fwd_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    bwd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev])) if cfg.backward and not graphs else None
 
     if rank != 0:
         if world > 1:
@@ -313,47 +387,59 @@ def run_ours(args):
         return
 
     # ---- roofline (algorithmic bytes / CUDA-event duration of the dominant call) ----
-    fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, g, aligned, fs)
-    ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz)
+    if g > 0:
+        fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, g, aligned, fs)
+        ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz)
+    else:   # adaptive grid: the touched set is at least the fixed-grid one; report the dense-pyramid bound instead
+        fp = {"level_hist": None}
+        ab = {"fwd": pyr_bytes * esz + K * C * PH * PW * esz + 20 * K, "bwd": K * C * PH * PW * esz + pyr_bytes * 4}
     peak, peak_src = peaks()
-    from paper_1906_07155_b200 import ncu_traffic
-    traffic = (ncu_traffic.TRAFFIC_BYTES.get(args.config, {})
-               if args.layout == "cl" and args.backward == "auto" and not args.no_reuse_prep else {})
-    legs = {"fwd": (ab["fwd"], fwd_ms)}
-    if bwd_ms is not None:
-        legs["bwd"] = (ab["bwd"], bwd_ms)
+    variant = f"{args.layout}:{args.backward}:{'reuse' if reuse else 'noreuse'}"
+    traffic, traffic_stale = ncu_traffic(args.config, variant)
+    legs = {"fwd": (ab["fwd"], loops["fwd"]["median_ms"])}
+    if cfg.backward:
+        legs["bwd"] = (ab["bwd"], loops["bwd"]["median_ms"])
     dom = max(legs, key=lambda k: legs[k][1])
+    NOMINAL = 8000.0
 
     def roof(name):
         by, ms = legs[name]
         ach = by / (ms * 1e-3) / 1e9
         return {"bound": "hbm", "kernel": name, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": traffic.get(name), "traffic_source": traffic.get("source"), "algorithmic_bytes": by, "ms": ms,
+                "frac_nominal_8000": ach / NOMINAL,
+                "traffic": traffic.get(name), "traffic_stale": bool(traffic_stale),
+                "traffic_source": "profiles/traffic.json (bench_traffic.py)" if traffic.get(name) else None,
+                "algorithmic_bytes": by, "ms": ms, "ms_min": loops[name]["min_ms"],
                 "peak_source": peak_src,
-                "note": "ms = CUDA-event time of the whole C-ABI call of this leg (fwd: gather kernel incl. the "
-                        "backward's prep blocks under RAF_REUSE_PREP; bwd: pull kernel, + its prep launch otherwise)"}
+                "note": "ms = median over windows of the CUDA-event time per C-ABI call of this leg run back to back "
+                        "(fwd: gather kernel incl. the backward's prep blocks under RAF_REUSE_PREP; bwd: pull "
+                        "kernel, + its prep launch otherwise); achieved = algorithmic bytes / ms"}
 
     step_ms = total_ms / args.steps
     step_bytes = ab["fwd"] + (ab["bwd"] if cfg.backward else 0)
+    step_ach = step_bytes / (step_ms * 1e-3) / 1e9
     line = {"metric": METRIC, "value": world * K / (step_ms * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: {cfg.name}", "K": K, "C": C,
-                       "out_size": [PH, PW], "levels": L, "layout": args.layout, "parallelism": f"replicas x{world} (shard by image, no collective)",
+                       "out_size": [PH, PW], "levels": L, "layout": args.layout, "sampling_ratio": g, "aligned": bool(aligned),
+                       "parallelism": f"{world} independent replica(s): every rank runs the whole workload on its own GPU "
+                                      "(the path shards by image; no collective)",
                        "l2_protocol": (f"inputs rotate over {R} independent copies ({R * ws_set / 1e6:.0f} MB >> L2 {l2 / 1e6:.0f} MB)"
                                        if R * ws_set >= 2 * l2 else
                                        f"WARM: {R} buffer set(s), {R * ws_set / 1e6:.0f} MB vs L2 {l2 / 1e6:.0f} MB (not the headline)"),
                        "backward": args.backward if cfg.backward else "none",
-                       "reuse_prep": bool(flags & B.RAF_REUSE_PREP) if cfg.backward else False,
-                       "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
+                       "reuse_prep": bool(reuse), "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
             "roofline": roof(dom),
-            "roofline_all": {k: roof(k) for k in legs} | {"step": {"achieved": step_bytes / (step_ms * 1e-3) / 1e9,
-                                                                  "frac": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
-                                                                  "algorithmic_bytes": step_bytes, "ms": step_ms}},
-            "clocks": clocks, "gpu_launches": int(launches)}
+            "roofline_all": {k: roof(k) for k in legs} | {"step": {
+                "achieved": step_ach, "frac": step_ach / peak, "frac_nominal_8000": step_ach / NOMINAL,
+                "algorithmic_bytes": step_bytes, "ms": step_ms,
+                "ms_window_median": loops["step"]["median_ms"], "ms_window_min": loops["step"]["min_ms"]}},
+            "loops": loops,
+            "clocks": clocks, "gpu_launches": int(launches), "source_hash": source_hash()}
 
     # ---- e2e: HOST buffers through the C ABI, copies inside the timed region ----
-    if not args.no_e2e:
+    if not args.no_e2e and g > 0:
         hf = [lay(f).pin_memory() if args.layout == "nchw" else f.permute(0, 2, 3, 1).contiguous().pin_memory().permute(0, 3, 1, 2)
               for f in base_feats]
         hrois = torch.from_numpy(wl.rois).pin_memory()
@@ -378,17 +464,17 @@ def run_ours(args):
         def e2e_step():
             B.roi_align_fpn_forward_host(hf, cfg.scales, hrois, hout, g, aligned, fs, arena, stream)
             if cfg.backward:
-                B.roi_align_fpn_backward_host(hgrads, cfg.scales, hgout, hrois, g, aligned, fs, flags, arena, stream)
+                B.roi_align_fpn_backward_host(hgrads, cfg.scales, hgout, hrois, g, aligned, fs, flags & ~B.RAF_REUSE_PREP, arena, stream)
         n_e2e = max(1, min(args.steps, 5))
         e2e_step()
         torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
         for _ in range(n_e2e):
             e2e_step()
-        e1.record(stream)
+        a1.record(stream)
         torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / n_e2e
+        ms = a0.elapsed_time(a1) / n_e2e
         line["e2e"] = {"value": world * K / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                        "d2h_bytes_per_step": int(d2h), "ms_per_step": ms, "steps": n_e2e,
                        "note": "roi_align_fpn_{forward,backward}_host: pinned host buffers, copies in the timed region"}

@@ -136,3 +136,29 @@ def test_product_does_not_import_oracle():
             text = open(os.path.join(ROOT, "oracle", fn)).read()
             assert "import paper_1906_07155_b200" not in text and "from paper_1906_07155_b200" not in text
             assert "libraf.so" not in text and "binding" not in text
+
+
+def test_binding_rejects_what_the_abi_cannot_see():
+    """binding.py validates dtypes / shapes / contiguity / devices before the raw pointers go down
+    (ValueError, no library call): the C ABI cannot see any of it."""
+    import torch
+    feats = [torch.zeros((1, 4, 8, 8)), torch.zeros((1, 4, 4, 4))]
+    rois = torch.zeros((3, 5))
+    out = torch.zeros((3, 4, 7, 7))
+    ws = torch.zeros(1024, dtype=torch.uint8)
+    scales = [0.25, 0.125]
+    call = lambda **kw: B.roi_align_fpn_forward(kw.get("feats", feats), scales, kw.get("rois", rois), kw.get("out", out),
+                                                2, True, 56.0, ws)
+    bad = [dict(rois=rois.double()), dict(rois=torch.zeros((3, 6))), dict(rois=torch.zeros((5, 3)).t()),
+           dict(rois=torch.zeros((4, 5))),                      # K differs from out
+           dict(out=torch.zeros((3, 8, 7, 7))),                 # C differs from the levels
+           dict(out=out.half()),                                # dtype differs from the features
+           dict(feats=[feats[0], torch.zeros((1, 8, 4, 4))]),   # C differs across levels
+           dict(feats=[feats[0], feats[1].half()]),
+           dict()]                                              # all valid but on the CPU: not CUDA tensors
+    for kw in bad:
+        with pytest.raises(ValueError):
+            call(**kw)
+    grads = [torch.zeros((1, 4, 8, 8)), torch.zeros((1, 4, 4, 4), dtype=torch.bfloat16)]
+    with pytest.raises(ValueError):   # gradient pyramid must be fp32
+        B.roi_align_fpn_backward(grads, scales, out, rois, 2, True, 56.0, 0, ws)

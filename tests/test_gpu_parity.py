@@ -319,11 +319,12 @@ def test_backward_full_size_config2(flags):
     cfg = wl.cfg
     got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl",
                                    "f32", flags)
-    # the oracle on a channel slice (channels are independent)
-    sl = slice(40, 56)
+    # the oracle on two channel slices, one in each 128-channel half of a lane's accumulators
+    # (channels are independent)
     shapes = [(s[0], 16, s[2], s[3]) for s in cfg.level_shapes]
-    ref, S = R.backward(shapes, cfg.scales, go_exact[:, sl], wl.rois, (7, 7), 2, True, 56.0)
-    T.assert_backward_close([g[:, sl] for g in got], ref, S)
+    for sl in (slice(40, 56), slice(224, 240)):
+        ref, S = R.backward(shapes, cfg.scales, go_exact[:, sl], wl.rois, (7, 7), 2, True, 56.0)
+        T.assert_backward_close([g[:, sl] for g in got], ref, S)
     # properties that hold at any size: total mass and untouched pixels
     masks = R.footprint(cfg.level_shapes, cfg.scales, wl.rois, (7, 7), 2, True)
     for g, m in zip(got, masks):
@@ -358,17 +359,121 @@ def test_full_size_step_as_benched(index):
     ref = R.forward(exact, cfg.scales, wl.rois[pick], (PH, PW), 2, True, cfg.finest_scale)
     T.assert_forward_close(out[torch.from_numpy(pick).cuda()].to(torch.float64).cpu().numpy(), ref, cfg.dtype)
     del exact
-    # backward, channel slice
-    sl = slice(96, 112)
+    # backward, two channel slices (one per 128-channel half)
     shapes = [(s_[0], 16, s_[2], s_[3]) for s_ in cfg.level_shapes]
-    gref, S = R.backward(shapes, cfg.scales, go_t[:, sl].to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
-                         cfg.finest_scale)
-    T.assert_backward_close([g[:, sl].to(torch.float64).cpu().numpy() for g in grads], gref, S)
+    for sl in (slice(96, 112), slice(224, 240)):
+        gref, S = R.backward(shapes, cfg.scales, go_t[:, sl].to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
+                             cfg.finest_scale)
+        T.assert_backward_close([g[:, sl].to(torch.float64).cpu().numpy() for g in grads], gref, S)
     masks = R.footprint(cfg.level_shapes, cfg.scales, wl.rois, (PH, PW), 2, True)
     for g, m in zip(grads, masks):
         assert bool(torch.isfinite(g).all())
         untouched = torch.from_numpy(m == 0).cuda()[:, None].expand_as(g)
         assert bool((g[untouched] == 0).all())
+
+
+def test_backward_full_size_config5_atomic():
+    """Config 5 at full size through the atomic variant (red.global.add.v4.f32), bf16 grad_out."""
+    wl = inputs.make_workload(5, with_feats=False)
+    cfg = wl.cfg
+    got, go_exact = T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, cfg.finest_scale, "cl",
+                                   "bf16", B.RAF_ATOMIC)
+    shapes = [(s[0], 8, s[2], s[3]) for s in cfg.level_shapes]
+    for sl in (slice(16, 24), slice(200, 208)):
+        ref, S = R.backward(shapes, cfg.scales, go_exact[:, sl], wl.rois, (7, 7), 2, True, cfg.finest_scale)
+        T.assert_backward_close([g[:, sl] for g in got], ref, S)
+
+
+def test_reuse_prep_with_foreign_workspace_is_loud():
+    """RAF_REUSE_PREP on a workspace that was NOT written for these arguments (forward on other RoIs, other
+    K, other geometry, or never written at all): the pull kernel compares the fingerprint the prep left and
+    poisons the whole gradient pyramid with NaN instead of computing from foreign tables."""
+    wl = inputs.make_workload(5, n_img=2, per_img=64, channels=32)
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    feats, _ = T.device_feats(wl.feats, "f32", "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    other = rois.clone()                       # same values, another buffer: a different RoI tensor
+    go = T.to_layout(torch.from_numpy(wl.grad_out).cuda(), "cl")
+    out = T.empty_layout((K, C, PH, PW), torch.float32, "cl")
+
+    def bwd(rois_t, ws, flags, g=2, aligned=True):
+        grads = [T.empty_layout(s, torch.float32, "cl", fill=1.0) for s in cfg.level_shapes]
+        B.roi_align_fpn_backward(grads, cfg.scales, go, rois_t, g, aligned, cfg.finest_scale, flags, ws)
+        torch.cuda.synchronize()
+        return grads
+
+    ws = T.workspace(K, L, PH, PW, 2)
+    B.roi_align_fpn_forward(feats, cfg.scales, rois, out, 2, True, cfg.finest_scale, ws)
+    good = bwd(rois, ws, B.RAF_REUSE_PREP)
+    assert all(bool(torch.isfinite(g).all()) for g in good)
+    for bad in (bwd(other, ws, B.RAF_REUSE_PREP),                       # forward ran on another RoI tensor
+                bwd(rois, ws, B.RAF_REUSE_PREP, aligned=False),         # other geometry
+                bwd(rois, T.workspace(K, L, PH, PW, 2), B.RAF_REUSE_PREP)):   # never written
+        assert all(bool(torch.isnan(g).all()) for g in bad)
+    # without the flag the same calls rebuild the tables and are fine
+    again = bwd(other, ws, 0)
+    for a_, b_ in zip(again, good):
+        assert torch.equal(a_, b_)
+
+
+def test_pull_prep_buckets_bit_exact():
+    """(a2) on the hot path: the (level, image) buckets the prep leaves in the workspace -- bperm / boff, read
+    back raw -- against a stable lexsort of the oracle's levels (unique answer -> bit-exact)."""
+    wl = inputs.make_workload(5, n_img=5, per_img=333, channels=8)
+    cfg = wl.cfg
+    rois_np = wl.rois.copy()
+    rois_np[7, 0] = -1.0        # invalid batch indices are dropped from the buckets
+    rois_np[100, 0] = 2.5
+    PH, PW = cfg.out_size
+    K, C, L, N = cfg.K, cfg.channels, len(cfg.level_shapes), cfg.n_img
+    feats, _ = T.device_feats(wl.feats, "f32", "cl")
+    rois = torch.from_numpy(rois_np).cuda()
+    out = T.empty_layout((K, C, PH, PW), torch.float32, "cl")
+    ws = T.workspace(K, L, PH, PW, 2)
+    B.roi_align_fpn_forward(feats, cfg.scales, rois, out, 2, True, cfg.finest_scale, ws)
+    torch.cuda.synchronize()
+    raw = ws.cpu().numpy()
+    align = lambda v: (v + 255) & ~255
+    o_bperm = 256
+    o_boff = o_bperm + align(4 * K)
+    bperm = raw[o_bperm:o_bperm + 4 * K].view(np.int32)
+    boff = raw[o_boff:o_boff + 4 * (L * N + 1)].view(np.int32)
+    levels = R.assign_levels(rois_np, L, cfg.finest_scale)[0]
+    b = rois_np[:, 0]
+    valid = (b >= 0) & (b < N) & (b == np.floor(b))
+    key = levels.astype(np.int64) * N + np.where(valid, b, 0).astype(np.int64)
+    ks = np.nonzero(valid)[0]
+    order = ks[np.argsort(key[ks], kind="stable")]
+    counts = np.bincount(key[ks], minlength=L * N)
+    assert np.array_equal(boff, np.concatenate([[0], np.cumsum(counts)]))
+    assert np.array_equal(bperm[:len(order)], order)
+
+
+def test_forward_ex_no_prep_and_workspace_checks():
+    """roi_align_fpn_forward_ex(RAF_NO_PREP): same values, the workspace is neither needed nor touched;
+    a misaligned workspace is refused."""
+    wl = inputs.make_workload(3, n_img=1, per_img=100, channels=64)
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    feats, _ = T.device_feats(wl.feats, "f16", "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    ws = T.workspace(K, L, PH, PW, 2)
+    o1 = T.empty_layout((K, C, PH, PW), torch.float16, "cl", fill=float("nan"))
+    o2 = T.empty_layout((K, C, PH, PW), torch.float16, "cl", fill=float("nan"))
+    B.roi_align_fpn_forward(feats, cfg.scales, rois, o1, 2, True, cfg.finest_scale, ws)
+    guard = ws.clone()
+    guard.fill_(0x5C)
+    B.roi_align_fpn_forward_ex(feats, cfg.scales, rois, o2, 2, True, cfg.finest_scale, B.RAF_NO_PREP, guard)
+    B.roi_align_fpn_forward_ex(feats, cfg.scales, rois, o2, 2, True, cfg.finest_scale, B.RAF_NO_PREP, None)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, o2)
+    assert bool((guard == 0x5C).all())
+    with pytest.raises(B.RafError) as e:
+        B.roi_align_fpn_forward(feats, cfg.scales, rois, o2, 2, True, cfg.finest_scale, ws[16:])
+    assert e.value.status == -6
 
 
 def test_adjoint_identity_on_gpu():

@@ -7,7 +7,8 @@ import numpy as np
 import pytest
 
 from oracle import raf_ref as R
-from paper_1906_07155_b200 import inputs, roofline, sharding
+import bench_roofline as roofline
+from paper_1906_07155_b200 import inputs, sharding
 
 
 @pytest.mark.parametrize("index", [2, 4])

@@ -11,18 +11,29 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "raf_ref.cpp")
 LIB = os.path.join(HERE, "libraf_ref.so")
+OPS_SRC = os.path.join(HERE, "ops_ref.cpp")      # RoIPool-max, NMS, Soft-NMS
+OPS_LIB = os.path.join(HERE, "libops_ref.so")
 FLAGS = ["-O2", "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared"]
 
 
-def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)
-            and os.path.getmtime(LIB) >= os.path.getmtime(__file__)):
-        return LIB
-    cmd = ["g++"] + FLAGS + [SRC, "-o", LIB + ".tmp"]
+def _build_one(src: str, lib: str, force: bool) -> str:
+    if (not force and os.path.exists(lib)
+            and os.path.getmtime(lib) >= os.path.getmtime(src)
+            and os.path.getmtime(lib) >= os.path.getmtime(__file__)):
+        return lib
+    cmd = ["g++"] + FLAGS + [src, "-o", lib + ".tmp"]
     subprocess.run(cmd, check=True)
-    os.replace(LIB + ".tmp", LIB)
-    return LIB
+    os.replace(lib + ".tmp", lib)
+    return lib
+
+
+def build(force: bool = False) -> str:
+    _build_one(OPS_SRC, OPS_LIB, force)
+    return _build_one(SRC, LIB, force)
+
+
+def build_ops(force: bool = False) -> str:
+    return _build_one(OPS_SRC, OPS_LIB, force)
 
 
 if __name__ == "__main__":

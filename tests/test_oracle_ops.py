@@ -1,0 +1,242 @@
+"""Pins of the CPU oracle for RoIPool-max, NMS and Soft-NMS (oracle/ops_ref.cpp, readings
+P1-P4 / N1-N6 of DESIGN.md 3b).  Nothing here touches the CUDA path; all -m "not gpu"."""
+import math
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import ops_ref as O
+
+
+# ------------------------------------------------------------------------------------------ RoIPool-max
+def _ramp(H, W, C=1, N=1):
+    f = (np.arange(H)[:, None] * W + np.arange(W)[None, :]).astype(np.float64)
+    return np.broadcast_to(f, (N, C, H, W)).copy()
+
+
+def _windows_exact(lo, hi, P, n):
+    """Bin windows of an INTEGER extent [lo, hi] (scale 1) in exact rational arithmetic."""
+    size = max(hi - lo + 1, 1)
+    b = Fraction(size, P)
+    out = []
+    for p in range(P):
+        s = math.floor(p * b) + lo
+        e = math.ceil((p + 1) * b) + lo
+        out.append((min(max(s, 0), n), min(max(e, 0), n)))
+    return out
+
+
+def test_roi_pool_integer_aligned_identity_and_block_max():
+    H = W = 16
+    f = _ramp(H, W)
+    # 7x7 pixels, 7x7 bins: every bin is one pixel -> identity crop
+    out, arg = O.roi_pool_forward([f], [1.0], np.array([[0, 2, 3, 8, 9]], np.float32), (7, 7))
+    assert np.array_equal(out[0, 0], f[0, 0, 3:10, 2:9])
+    assert np.array_equal(arg[0, 0], (np.arange(3, 10)[:, None] * W + np.arange(2, 9)[None, :]))
+    # 14x14 pixels, 7x7 bins: 2x2 blocks, max of an increasing ramp = bottom-right pixel of the block
+    out, arg = O.roi_pool_forward([f], [1.0], np.array([[0, 0, 0, 13, 13]], np.float32), (7, 7))
+    assert np.array_equal(out[0, 0], f[0, 0, 1:14:2, 1:14:2])
+    # on the negated ramp the FIRST pixel of the block wins: the window start is pinned too
+    out, arg = O.roi_pool_forward([-f], [1.0], np.array([[0, 0, 0, 13, 13]], np.float32), (7, 7))
+    assert np.array_equal(out[0, 0], -f[0, 0, 0:14:2, 0:14:2])
+
+
+def test_roi_pool_windows_match_exact_rational_arithmetic():
+    """Random integer boxes (scale 1, so quantisation is exact): the window of every bin, read back from the
+    argmax on an increasing ramp (last pixel) and on a decreasing ramp (first pixel), equals the window
+    computed with exact fractions -- including boxes partly or wholly outside the map and empty bins."""
+    rng = np.random.default_rng(7)
+    H, W = 20, 24
+    f = _ramp(H, W)
+    for P in ((7, 7), (3, 5), (14, 14)):
+        for _ in range(60):
+            x1, y1 = int(rng.integers(-6, W)), int(rng.integers(-6, H))
+            x2, y2 = x1 + int(rng.integers(0, 22)), y1 + int(rng.integers(0, 22))
+            roi = np.array([[0, x1, y1, x2, y2]], np.float32)
+            up, au = O.roi_pool_forward([f], [1.0], roi, P)
+            dn, ad = O.roi_pool_forward([-f], [1.0], roi, P)
+            wy = _windows_exact(y1, y2, P[0], H)
+            wx = _windows_exact(x1, x2, P[1], W)
+            for ph, (hs, he) in enumerate(wy):
+                for pw, (ws, we) in enumerate(wx):
+                    if he <= hs or we <= ws:
+                        assert au[0, 0, ph, pw] == -1 and up[0, 0, ph, pw] == 0.0
+                    else:
+                        assert au[0, 0, ph, pw] == (he - 1) * W + (we - 1)
+                        assert ad[0, 0, ph, pw] == hs * W + ws
+                        assert up[0, 0, ph, pw] == f[0, 0, he - 1, we - 1]
+
+
+def test_roi_pool_rounding_of_scaled_corners():
+    """roundf (half away from zero) of x*scale decides the window: 2.5 -> 3, 3.49 -> 3, -0.5 -> -1."""
+    f = _ramp(12, 12)
+    # scale 0.25: x1 = 10 -> 2.5 -> 3 ; x2 = 22 -> 5.5 -> 6 ; one bin -> whole window [3, 6]
+    out, arg = O.roi_pool_forward([-f], [0.25], np.array([[0, 10, 10, 22, 22]], np.float32), (1, 1))
+    assert arg[0, 0, 0, 0] == 3 * 12 + 3
+    out, arg = O.roi_pool_forward([f], [0.25], np.array([[0, 10, 10, 22, 22]], np.float32), (1, 1))
+    assert arg[0, 0, 0, 0] == 6 * 12 + 6
+    out, arg = O.roi_pool_forward([-f], [0.25], np.array([[0, 13.96, 13.96, 22, 22]], np.float32), (1, 1))
+    assert arg[0, 0, 0, 0] == 3 * 12 + 3          # 3.49 -> 3
+    out, arg = O.roi_pool_forward([-f], [1.0], np.array([[0, -0.5, -0.5, 3, 3]], np.float32), (1, 1))
+    assert arg[0, 0, 0, 0] == 0                    # -0.5 -> -1, clamped to 0
+
+
+def test_roi_pool_constant_ties_invalid_and_levels():
+    c = np.full((2, 3, 8, 8), 2.5)
+    out, arg = O.roi_pool_forward([c], [1.0], np.array([[1, 1, 1, 5, 6], [7, 1, 1, 5, 6], [0.5, 1, 1, 5, 6]], np.float32), (3, 3))
+    assert np.all(out[0] == 2.5) and np.all(out[1:] == 0) and np.all(arg[1:] == -1)
+    # ties: the FIRST maximum in row-major order
+    assert arg[0, 0, 0, 0] == 1 * 8 + 1
+    # NaN never wins; an all-NaN window yields 0 / -1
+    d = c.copy(); d[0, 0, 2, 2] = np.nan
+    out, arg = O.roi_pool_forward([d], [1.0], np.array([[0, 2, 2, 2, 2]], np.float32), (1, 1))
+    assert out[0, 0, 0, 0] == 0 and arg[0, 0, 0, 0] == -1 and out[0, 1, 0, 0] == 2.5
+    # level routing: side 50 -> level 0 (scale 1/4), side 300 -> level 2 (scale 1/16), finest_scale 56
+    feats = [np.full((1, 1, 64, 64), float(l)) for l in range(4)]
+    scales = [1 / 4, 1 / 8, 1 / 16, 1 / 32]
+    out, _ = O.roi_pool_forward(feats, scales, np.array([[0, 10, 10, 60, 60], [0, 10, 10, 310, 310]], np.float32), (2, 2))
+    assert np.all(out[0] == 0.0) and np.all(out[1] == 2.0)
+
+
+def test_roi_pool_matches_library_routine():
+    tv = pytest.importorskip("torchvision")
+    import torch
+    rng = np.random.default_rng(11)
+    for scale, P in ((1.0, (7, 7)), (0.25, (7, 7)), (0.5, (3, 5))):
+        f = rng.standard_normal((2, 3, 24, 30))
+        K = 60
+        x1 = rng.uniform(-5, 30 / scale, K); y1 = rng.uniform(-5, 24 / scale, K)
+        w = rng.uniform(0, 25 / scale, K); h = rng.uniform(0, 25 / scale, K)
+        rois = np.stack([rng.integers(0, 2, K), x1, y1, x1 + w, y1 + h], 1).astype(np.float32)
+        out, _ = O.roi_pool_forward([f], [scale], rois, P, finest_scale=1e9)
+        ref = tv.ops.roi_pool(torch.from_numpy(f), torch.from_numpy(rois).double(), P, scale).numpy()
+        assert np.array_equal(out, ref)
+
+
+def test_roi_pool_backward_is_the_transpose_of_the_selection():
+    rng = np.random.default_rng(5)
+    shapes = [(2, 3, 20, 28), (2, 3, 10, 14)]
+    feats = [rng.standard_normal(s) for s in shapes]
+    scales = [0.25, 0.125]
+    K = 40
+    side = np.exp(rng.uniform(np.log(8), np.log(200), K))
+    cx, cy = rng.uniform(0, 112, K), rng.uniform(0, 80, K)
+    rois = np.stack([rng.integers(0, 2, K), cx - side / 2, cy - side / 2, cx + side / 2, cy + side / 2], 1).astype(np.float32)
+    out, arg = O.roi_pool_forward(feats, scales, rois, (7, 7))
+    g = rng.standard_normal(out.shape)
+    grads = O.roi_pool_backward(shapes, scales, g, arg, rois)
+    # <pool(x), g> = <x, pool^T g> (the forward is x[argmax])
+    lhs = float((out * g).sum())
+    rhs = float(sum((f * gr).sum() for f, gr in zip(feats, grads)))
+    assert abs(lhs - rhs) <= 1e-12 * max(1.0, abs(lhs))
+    # mass: every valid bin delivers its gradient exactly once
+    assert abs(sum(gr.sum() for gr in grads) - g[arg >= 0].sum()) < 1e-10
+    # brute force with numpy scatter
+    from oracle import raf_ref as R
+    lv = R.assign_levels(rois, 2, 56.0)[0]
+    want = [np.zeros(s) for s in shapes]
+    for k in range(K):
+        b = int(rois[k, 0])
+        flat = want[lv[k]][b].reshape(3, -1)
+        for c in range(3):
+            m = arg[k, c] >= 0
+            np.add.at(flat[c], arg[k, c][m], g[k, c][m])
+    for a_, b_ in zip(grads, want):
+        assert np.allclose(a_, b_, rtol=0, atol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------- NMS
+def test_iou_closed_forms():
+    assert O.iou([0, 0, 2, 2], [0, 0, 2, 2]) == 1.0
+    assert O.iou([0, 0, 2, 2], [2, 0, 4, 2]) == 0.0            # touching edges
+    assert O.iou([0, 0, 2, 2], [5, 5, 6, 6]) == 0.0
+    assert O.iou([0, 0, 4, 4], [1, 1, 3, 3]) == np.float32(4) / np.float32(16)     # contained: area ratio
+    assert O.iou([0, 0, 2, 2], [1, 1, 3, 3]) == np.float32(np.float32(1) / np.float32(7))
+    assert O.iou([0, 0, 2, 2], [1, 1, 3, 3]) == O.iou([1, 1, 3, 3], [0, 0, 2, 2])
+    assert math.isnan(O.iou([1, 1, 1, 1], [1, 1, 1, 1]))       # 0/0: compares false everywhere
+
+
+def test_nms_worked_example_and_threshold_edge():
+    boxes = np.array([[0, 0, 10, 10], [1, 1, 11, 11], [20, 20, 30, 30], [0, 0, 10, 9], [21, 21, 29, 29]], np.float32)
+    scores = np.array([0.9, 0.8, 0.7, 0.95, 0.1], np.float32)
+    # order: 3, 0, 1, 2, 4.  IoU(3,0) = 90/100 = 0.9 -> 0 out; IoU(3,1) = 72/(90+100-72) = 0.61 -> 1 out;
+    # 2 kept; IoU(2,4) = 64/100 = 0.64 -> 4 out at threshold 0.5
+    assert O.nms(boxes, scores, 0.5).tolist() == [3, 2]
+    assert O.nms(boxes, scores, 0.62).tolist() == [3, 1, 2]      # 0.61 no longer suppresses 1; 0.64 still suppresses 4
+    assert O.nms(boxes, scores, 0.65).tolist() == [3, 1, 2, 4]   # (0 stays out: IoU(3,0) = 0.9)
+    assert O.nms(boxes, scores, 0.95).tolist() == [3, 0, 1, 2, 4]
+    # strict comparison: IoU == threshold is kept
+    b = np.array([[0, 0, 2, 2], [0, 0, 2, 1]], np.float32)
+    assert O.nms(b, np.array([0.9, 0.8], np.float32), 0.5).tolist() == [0, 1]
+    assert O.nms(b, np.array([0.9, 0.8], np.float32), 0.49).tolist() == [0]
+    # ties in score: lower index first; empty input
+    assert O.nms(boxes[[2, 2, 2]], np.array([0.5, 0.5, 0.5], np.float32), 0.5).tolist() == [0]
+    assert O.nms(np.zeros((0, 4), np.float32), np.zeros(0, np.float32), 0.5).tolist() == []
+
+
+def _random_boxes(rng, n, span=200.0):
+    side = np.exp(rng.uniform(np.log(8), np.log(120), n))
+    asp = np.exp(rng.uniform(np.log(0.5), np.log(2), n))
+    w, h = side * np.sqrt(asp), side / np.sqrt(asp)
+    cx, cy = rng.uniform(0, span, n), rng.uniform(0, span, n)
+    return np.stack([cx - w / 2, cy - h / 2, cx + w / 2, cy + h / 2], 1).astype(np.float32)
+
+
+def test_nms_matches_library_routine_and_invariants():
+    rng = np.random.default_rng(3)
+    for n, thr in ((50, 0.5), (300, 0.7), (400, 0.3)):
+        boxes = _random_boxes(rng, n)
+        scores = rng.permutation(n).astype(np.float32) / n          # distinct
+        keep = O.nms(boxes, scores, thr)
+        # kept boxes do not suppress each other; every dropped box is suppressed by a kept, higher-scored one
+        for i, a in enumerate(keep):
+            for b in keep[i + 1:]:
+                assert not (O.iou(boxes[a], boxes[b]) > thr)
+        kept = set(keep.tolist())
+        for j in range(n):
+            if j not in kept:
+                assert any(scores[a] > scores[j] and O.iou(boxes[a], boxes[j]) > thr for a in keep)
+        assert np.all(np.diff(scores[keep]) < 0)
+        # idempotent, and invariant under a permutation of the input
+        assert O.nms(boxes[keep], scores[keep], thr).tolist() == list(range(len(keep)))
+        perm = rng.permutation(n)
+        assert sorted(perm[O.nms(boxes[perm], scores[perm], thr)].tolist()) == sorted(keep.tolist())
+    tv = pytest.importorskip("torchvision")
+    import torch
+    boxes = _random_boxes(rng, 500)
+    scores = rng.permutation(500).astype(np.float32) / 500
+    ref = tv.ops.nms(torch.from_numpy(boxes), torch.from_numpy(scores), 0.5).numpy()
+    assert O.nms(boxes, scores, 0.5).tolist() == ref.tolist()
+
+
+# ------------------------------------------------------------------------------------------ Soft-NMS
+def test_soft_nms_worked_examples():
+    boxes = np.array([[0, 0, 2, 2], [1, 0, 3, 2], [10, 10, 11, 11]], np.float32)   # IoU(0,1) = 2/6 = 1/3
+    scores = np.array([0.9, 0.8, 0.5], np.float32)
+    idx, sc = O.soft_nms(boxes, scores, 0.3, 0.5, 0.001, "linear")
+    assert idx.tolist() == [0, 1, 2]
+    assert np.allclose(sc, [0.9, 0.8 * (1 - 1 / 3), 0.5], rtol=1e-6)
+    idx, sc = O.soft_nms(boxes, scores, 0.3, 0.5, 0.001, "gaussian")
+    assert idx.tolist() == [0, 1, 2]
+    assert np.allclose(sc, [0.9, 0.8 * math.exp(-(1 / 9) / 0.5), 0.5], rtol=1e-6)
+    # below the IoU threshold the linear method leaves the score alone
+    idx, sc = O.soft_nms(boxes, scores, 0.4, 0.5, 0.001, "linear")
+    assert np.allclose(sc, [0.9, 0.8, 0.5])
+    # the decayed score decides the order: 0.8 * (1 - 1/3) = 0.533 drops below an untouched 0.6
+    idx, sc = O.soft_nms(boxes, np.array([0.9, 0.8, 0.6], np.float32), 0.3, 0.5, 0.001, "linear")
+    assert idx.tolist() == [0, 2, 1]
+    # min_score prunes
+    idx, sc = O.soft_nms(boxes, scores, 0.3, 0.5, 0.52, "linear")
+    assert idx.tolist() == [0, 1]
+
+
+def test_soft_nms_without_overlap_is_a_score_sort():
+    rng = np.random.default_rng(9)
+    n = 40
+    boxes = np.stack([np.arange(n) * 10.0, np.zeros(n), np.arange(n) * 10.0 + 5, np.full(n, 5.0)], 1).astype(np.float32)
+    scores = rng.uniform(0.1, 1, n).astype(np.float32)
+    for method in ("linear", "gaussian"):
+        idx, sc = O.soft_nms(boxes, scores, 0.3, 0.5, 0.0, method)
+        assert idx.tolist() == np.argsort(-scores, kind="stable").tolist()
+        assert np.array_equal(sc, scores[idx])

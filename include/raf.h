@@ -121,6 +121,47 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                            int K, int out_h, int out_w, int sampling_ratio, int aligned,
                            float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream);
 
+/* ---- the max variant of the "RoIPooling-like operators" (the RoI pooling
+ * layer of Fast R-CNN), on the same FPN level map (C1) -------------------------------------------
+ * Window of bin (ph,pw) on the RoI's level (fp32, each operation rounded; readings P1-P4):
+ *   sw = roundf(x1*scale), ew = roundf(x2*scale), rw = max(ew - sw + 1, 1), bw = rw / out_w,
+ *   ws = clamp(floorf(pw*bw) + sw, 0, W), we = clamp(ceilf((pw+1)*bw) + sw, 0, W); rows likewise.
+ * out = max of the features over the window (0 for an empty window or an invalid batch index);
+ * argmax (int32 DEVICE, same logical shape and strides as `out`; may be NULL) = y*W + x of the FIRST maximum
+ * in row-major order, -1 when there is none.  NaN never wins.  Values are copies of inputs: exact. */
+int roi_pool_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                         int out_h, int out_w, float finest_scale, void* out, int32_t* argmax,
+                         const int64_t* out_strides, void* stream);
+
+/* Backward of RoIPool-max: grad_feats[level_k][b_k][c][argmax] += grad_out[k,c,ph,pw] (fp32 atomics: the
+ * summation order is not fixed).  grad_feats is zero-filled first unless RAF_ACCUMULATE (the only flag
+ * accepted).  argmax: what roi_pool_fpn_forward wrote for the same rois, addressed through gout_strides;
+ * entries that are not a pixel index of the RoI's level are ignored. */
+int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype, const void* grad_out,
+                          const int32_t* argmax, const int64_t* gout_strides, const float* rois, int K,
+                          int out_h, int out_w, float finest_scale, int flags, void* stream);
+
+/* ---- NMS and Soft-NMS on the GPU ("Soft NMS [1]: an alternative to NMS", PAPER.md:55;
+ * "All basic bbox and mask operations run on GPUs") ---------------------------------------------
+ * boxes: float32 DEVICE [n,4] = (x1,y1,x2,y2), continuous coordinates (no "+1"); scores: float32 DEVICE [n],
+ * no NaN.  IoU = inter / ((area_a + area_b) - inter), fp32, each operation rounded (readings N1-N6).
+ * Greedy NMS: boxes in descending score (ties: lower index first); a box is dropped when an earlier KEPT box
+ * has IoU > iou_threshold (strict).  keep[n] int32 DEVICE receives the kept indices in that order,
+ * num_keep[1] int32 DEVICE their number.  n <= 65536.  ws: roi_nms_workspace_bytes(n) bytes, 256-aligned. */
+size_t roi_nms_workspace_bytes(int n);
+int roi_nms(const float* boxes, const float* scores, int n, float iou_threshold, int32_t* keep,
+            int32_t* num_keep, void* ws, size_t ws_bytes, void* stream);
+
+/* Soft-NMS: repeatedly emit the remaining box of highest current score (ties: lowest index) and decay every
+ * other remaining score by  method RAF_SOFT_LINEAR: (iou > iou_threshold ? 1 - iou : 1),
+ * RAF_SOFT_GAUSSIAN: exp(-iou*iou / sigma);  boxes whose score falls below min_score are dropped.
+ * keep[n] / new_scores[n] in emission order, num_keep[1] their number.  n <= 8192 (one CTA, scores in
+ * shared memory).  The Gaussian method uses expf: scores agree with a host evaluation to a few ulp. */
+enum { RAF_SOFT_LINEAR = 1, RAF_SOFT_GAUSSIAN = 2 };
+int roi_soft_nms(const float* boxes, const float* scores, int n, float iou_threshold, float sigma,
+                 float min_score, int method, int32_t* keep, float* new_scores, int32_t* num_keep,
+                 void* ws, size_t ws_bytes, void* stream);
+
 /* End-to-end variants with HOST buffers (used for the e2e benchmark line): every `data` pointer in
  * the descriptors, `rois`, `out` / `grad_out` are HOST pointers (pinned for full copy speed) and
  * must be contiguous in the order the strides describe (each level / tensor occupies exactly

@@ -16,12 +16,14 @@ LIB_PATH = os.path.join(HERE, "libraf.so")
 
 RAF_F32, RAF_F16, RAF_BF16 = 0, 1, 2
 RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC, RAF_REUSE_PREP, RAF_NO_PREP = 1, 2, 4, 8, 16
+RAF_SOFT_LINEAR, RAF_SOFT_GAUSSIAN = 1, 2
 _DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_BF16}
 
 EXPORTS = [
     "roi_align_fpn_workspace_bytes", "roi_fpn_assign_levels", "roi_align_fpn_forward",
     "roi_align_fpn_forward_ex", "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
+    "roi_pool_fpn_forward", "roi_pool_fpn_backward", "roi_nms_workspace_bytes", "roi_nms", "roi_soft_nms",
 ]
 
 
@@ -70,6 +72,17 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = args
         L.roi_align_fpn_forward_ex.restype = ctypes.c_int
         L.roi_align_fpn_forward_ex.argtypes = fwd_args[:12] + [ctypes.c_int] + fwd_args[12:]
+        vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
+        L.roi_pool_fpn_forward.restype = ci
+        L.roi_pool_fpn_forward.argtypes = [vp, ci, ci, vp, ci, ci, ci, cf, vp, vp, vp, vp]
+        L.roi_pool_fpn_backward.restype = ci
+        L.roi_pool_fpn_backward.argtypes = [vp, ci, ci, vp, vp, vp, vp, ci, ci, ci, cf, ci, vp]
+        L.roi_nms_workspace_bytes.restype = ctypes.c_size_t
+        L.roi_nms_workspace_bytes.argtypes = [ci]
+        L.roi_nms.restype = ci
+        L.roi_nms.argtypes = [vp, vp, ci, cf, vp, vp, vp, ctypes.c_size_t, vp]
+        L.roi_soft_nms.restype = ci
+        L.roi_soft_nms.argtypes = [vp, vp, ci, cf, cf, cf, ci, vp, vp, vp, vp, ctypes.c_size_t, vp]
         L.roi_align_fpn_strerror.restype = ctypes.c_char_p
         L.roi_align_fpn_strerror.argtypes = [ctypes.c_int]
         L.roi_align_fpn_launch_count.restype = ctypes.c_uint64
@@ -247,3 +260,74 @@ def roi_align_fpn_backward_host(grad_feats_host: Sequence[torch.Tensor], scales,
                                            _stream_ptr(stream))
     if rc:
         raise RafError(rc, "roi_align_fpn_backward_host")
+
+
+# ---- RoIPool-max, NMS, Soft-NMS -------------------------------------------------------------
+def roi_pool_fpn_forward(feats: Sequence[torch.Tensor], scales: Sequence[float], rois: torch.Tensor,
+                         out: torch.Tensor, argmax: Optional[torch.Tensor], finest_scale: float, stream=None) -> None:
+    """out: logical [K,C,PH,PW]; argmax: int32 tensor of the same shape AND strides as `out` (or None)."""
+    _check_call(feats, feats[0].dtype if len(feats) else None, rois, out, feats[0].dtype if len(feats) else None, None)
+    if feats[0].dtype not in _DTYPES:
+        raise ValueError(f"unsupported feature dtype {feats[0].dtype}")
+    if argmax is not None and (argmax.dtype != torch.int32 or argmax.shape != out.shape or argmax.stride() != out.stride()
+                               or argmax.device != out.device):
+        raise ValueError("argmax must be an int32 tensor with the shape, strides and device of out")
+    K, _, PH, PW = out.shape
+    rc = lib().roi_pool_fpn_forward(make_levels(feats, scales), len(feats), _DTYPES[feats[0].dtype], _ptr(rois), K, PH, PW,
+                                    finest_scale, _ptr(out), _ptr(argmax), _strides4(out), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_pool_fpn_forward")
+
+
+def roi_pool_fpn_backward(grad_feats: Sequence[torch.Tensor], scales: Sequence[float], grad_out: torch.Tensor,
+                          argmax: torch.Tensor, rois: torch.Tensor, finest_scale: float, flags: int = 0, stream=None) -> None:
+    if grad_out.dtype not in _DTYPES:
+        raise ValueError(f"unsupported grad_out dtype {grad_out.dtype}")
+    _check_call(grad_feats, torch.float32, rois, grad_out, grad_out.dtype, None)
+    if (argmax.dtype != torch.int32 or argmax.shape != grad_out.shape or argmax.stride() != grad_out.stride()
+            or argmax.device != grad_out.device):
+        raise ValueError("argmax must be an int32 tensor with the shape, strides and device of grad_out")
+    K, _, PH, PW = grad_out.shape
+    rc = lib().roi_pool_fpn_backward(make_levels(grad_feats, scales), len(grad_feats), _DTYPES[grad_out.dtype], _ptr(grad_out),
+                                     _ptr(argmax), _strides4(grad_out), _ptr(rois), K, PH, PW, finest_scale, int(flags),
+                                     _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_pool_fpn_backward")
+
+
+def _check_boxes(boxes: torch.Tensor, scores: torch.Tensor) -> int:
+    if boxes.dtype != torch.float32 or boxes.dim() != 2 or boxes.shape[1] != 4 or not boxes.is_contiguous():
+        raise ValueError("boxes must be a contiguous float32 [n,4] tensor")
+    if scores.dtype != torch.float32 or scores.dim() != 1 or scores.shape[0] != boxes.shape[0] or not scores.is_contiguous():
+        raise ValueError("scores must be a contiguous float32 [n] tensor")
+    if not (boxes.is_cuda and scores.is_cuda and boxes.device == scores.device):
+        raise ValueError("boxes and scores must live on the same CUDA device")
+    return boxes.shape[0]
+
+
+def roi_nms_workspace_bytes(n: int) -> int:
+    return int(lib().roi_nms_workspace_bytes(int(n)))
+
+
+def roi_nms(boxes: torch.Tensor, scores: torch.Tensor, iou_threshold: float, keep: torch.Tensor, num_keep: torch.Tensor,
+            ws: Optional[torch.Tensor], stream=None) -> None:
+    """keep: int32 [n] device, num_keep: int32 [1] device (the caller reads it when it needs the count)."""
+    n = _check_boxes(boxes, scores)
+    if keep.dtype != torch.int32 or keep.numel() < n or num_keep.dtype != torch.int32 or not keep.is_cuda or not num_keep.is_cuda:
+        raise ValueError("keep must be int32 [n] and num_keep int32 [1], on the device")
+    rc = lib().roi_nms(_ptr(boxes), _ptr(scores), n, float(iou_threshold), _ptr(keep), _ptr(num_keep), _ptr(ws),
+                       0 if ws is None else ws.numel() * ws.element_size(), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_nms")
+
+
+def roi_soft_nms(boxes: torch.Tensor, scores: torch.Tensor, iou_threshold: float, sigma: float, min_score: float,
+                 method: int, keep: torch.Tensor, new_scores: torch.Tensor, num_keep: torch.Tensor, stream=None) -> None:
+    n = _check_boxes(boxes, scores)
+    if (keep.dtype != torch.int32 or keep.numel() < n or new_scores.dtype != torch.float32 or new_scores.numel() < n
+            or num_keep.dtype != torch.int32 or not (keep.is_cuda and new_scores.is_cuda and num_keep.is_cuda)):
+        raise ValueError("keep int32 [n], new_scores float32 [n], num_keep int32 [1], on the device")
+    rc = lib().roi_soft_nms(_ptr(boxes), _ptr(scores), n, float(iou_threshold), float(sigma), float(min_score), int(method),
+                            _ptr(keep), _ptr(new_scores), _ptr(num_keep), None, 0, _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_soft_nms")

@@ -279,6 +279,97 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   return launch_backward_atomic(p, gout_dtype, a, grad_out, gout_strides, cl, st);
 }
 
+// ---- RoIPool-max -------------------------------------------------------------------------------------
+static bool unit_channel_stride(const raf_level* lv, int L) {
+  for (int l = 0; l < L; ++l)
+    if (lv[l].sc != 1) return false;
+  return true;
+}
+
+static int zero_fill(const raf_level* grad_feats, int L, cudaStream_t st) {
+  for (int l = 0; l < L; ++l) {
+    const raf_level& v = grad_feats[l];
+    if (level_dense(v)) {
+      if (cudaMemsetAsync(v.data, 0, sizeof(float) * (size_t)v.n * v.c * v.h * v.w, st) != cudaSuccess) return RAF_ERR_CUDA;
+      count_launch();
+    } else {
+      const int rc = launch_zero_level((float*)v.data, v.n, v.c, v.h, v.w, v.sn, v.sc, v.sh, v.sw, st);
+      if (rc) return rc;
+    }
+  }
+  return RAF_OK;
+}
+
+int roi_pool_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                         int out_h, int out_w, float finest_scale, void* out, int32_t* argmax,
+                         const int64_t* out_strides, void* stream) {
+  int rc = check_levels(feats, L);
+  if (rc) return rc;
+  rc = check_common(rois, K, out_h, out_w, 1);
+  if (rc) return rc;
+  if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
+  if (!out_strides) return RAF_ERR_NULL;
+  if (K == 0) return RAF_OK;
+  for (int i = 0; i < 4; ++i) if (out_strides[i] <= 0) return RAF_ERR_STRIDE;
+  if (!out) return RAF_ERR_NULL;
+  for (int l = 0; l < L; ++l)
+    if ((int64_t)feats[l].h * feats[l].w >= ((int64_t)1 << 31)) return RAF_ERR_UNSUPPORTED;   // argmax is int32
+  LevelsParam p;
+  fill_param(feats, L, &p);
+  return launch_pool_forward(p, dtype, rois, K, out_h, out_w, finest_scale, out, argmax, out_strides,
+                             unit_channel_stride(feats, L), (cudaStream_t)stream);
+}
+
+int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype, const void* grad_out,
+                          const int32_t* argmax, const int64_t* gout_strides, const float* rois, int K,
+                          int out_h, int out_w, float finest_scale, int flags, void* stream) {
+  int rc = check_levels(grad_feats, L);
+  if (rc) return rc;
+  rc = check_common(rois, K, out_h, out_w, 1);
+  if (rc) return rc;
+  if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
+  if (flags & ~RAF_ACCUMULATE) return RAF_ERR_UNSUPPORTED;
+  if (!gout_strides) return RAF_ERR_NULL;
+  for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
+  if (K > 0 && (!grad_out || !argmax)) return RAF_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!(flags & RAF_ACCUMULATE)) {
+    rc = zero_fill(grad_feats, L, st);
+    if (rc) return rc;
+  }
+  if (K == 0) return RAF_OK;
+  LevelsParam p;
+  fill_param(grad_feats, L, &p);
+  return launch_pool_backward(p, gout_dtype, rois, K, out_h, out_w, finest_scale, grad_out, argmax, gout_strides,
+                              unit_channel_stride(grad_feats, L), st);
+}
+
+// ---- NMS / Soft-NMS ------------------------------------------------------------------------------------
+size_t roi_nms_workspace_bytes(int n) { return nms_workspace_bytes(n > 0 ? n : 0); }
+
+int roi_nms(const float* boxes, const float* scores, int n, float iou_threshold, int32_t* keep,
+            int32_t* num_keep, void* ws, size_t ws_bytes, void* stream) {
+  if (n < 0 || n > 65536) return RAF_ERR_SHAPE;
+  if (!num_keep || (n > 0 && (!boxes || !scores || !keep))) return RAF_ERR_NULL;
+  if (n > 0 && !ws) return RAF_ERR_NULL;
+  if (n > 0 && (((uintptr_t)ws % 256) || ws_bytes < nms_workspace_bytes(n))) return RAF_ERR_WORKSPACE;
+  return launch_nms(boxes, scores, n, iou_threshold, keep, num_keep, ws, (cudaStream_t)stream);
+}
+
+int roi_soft_nms(const float* boxes, const float* scores, int n, float iou_threshold, float sigma,
+                 float min_score, int method, int32_t* keep, float* new_scores, int32_t* num_keep,
+                 void* ws, size_t ws_bytes, void* stream) {
+  (void)ws; (void)ws_bytes;
+  if (n < 0 || n > 8192) return RAF_ERR_SHAPE;
+  if (method != RAF_SOFT_LINEAR && method != RAF_SOFT_GAUSSIAN) return RAF_ERR_UNSUPPORTED;
+  if (method == RAF_SOFT_GAUSSIAN && !(sigma > 0.0f)) return RAF_ERR_SHAPE;
+  if (!num_keep || (n > 0 && (!boxes || !scores || !keep || !new_scores))) return RAF_ERR_NULL;
+  return launch_soft_nms(boxes, scores, n, iou_threshold, sigma, min_score, method, keep, new_scores, num_keep, ws,
+                         (cudaStream_t)stream);
+}
+
 // ---- end-to-end variants with HOST buffers -----------------------------------------------------
 static bool tensor_dense(int K, int C, int PH, int PW, const int64_t* s) {
   raf_level v;

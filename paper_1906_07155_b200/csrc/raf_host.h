@@ -60,6 +60,20 @@ int pull_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a
 int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
                          const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream);
 
+// RoIPool-max (raf_pool.cu).  `chan_fastest`: enumerate outputs with the channel fastest (channels-last
+// features: coalesced window loads).  The gradient pyramid must already hold its starting values.
+int launch_pool_forward(const LevelsParam& lv, raf_dtype dtype, const float* rois, int K, int PH, int PW, float fs,
+                        void* out, int32_t* argmax, const int64_t* os, bool chan_fastest, cudaStream_t stream);
+int launch_pool_backward(const LevelsParam& glv, raf_dtype dtype, const float* rois, int K, int PH, int PW, float fs,
+                         const void* gout, const int32_t* argmax, const int64_t* gs, bool chan_fastest, cudaStream_t stream);
+
+// NMS / Soft-NMS (raf_nms.cu).
+size_t nms_workspace_bytes(int n);
+int launch_nms(const float* boxes, const float* scores, int n, float iou_threshold, int32_t* keep, int32_t* num_keep,
+               void* ws, cudaStream_t stream);
+int launch_soft_nms(const float* boxes, const float* scores, int n, float iou_threshold, float sigma, float min_score,
+                    int method, int32_t* keep, float* new_scores, int32_t* num_keep, void* ws, cudaStream_t stream);
+
 // Zero-fill of one strided level (used when the level is not one dense block).
 int launch_zero_level(float* data, int n, int c, int h, int w, int64_t sn, int64_t sc, int64_t sh,
                       int64_t sw, cudaStream_t stream);

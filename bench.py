@@ -45,6 +45,10 @@ def parse_args():
     ap.add_argument("--rotate", type=int, default=0,
                     help="number of independent input/output buffer sets to rotate over (0 = cold-L2 protocol: "
                          "at least 4 and >= 2x L2; 1 = WARM single-buffer number, not the headline)")
+    ap.add_argument("--op", default="align", choices=["align", "pool", "nms", "softnms"],
+                    help="align: the headline FPN RoIAlign fwd+bwd (BASELINE.json metric); pool / nms / softnms: the SURVEY 8(f) "
+                         "operations, one extra bench line each (not the headline)")
+    ap.add_argument("--nms-n", type=int, default=2000, help="boxes for --op nms / softnms")
     ap.add_argument("--windows", type=int, default=5, help="timing windows per loop (median and min are reported)")
     ap.add_argument("--window-iters", type=int, default=200, help="back-to-back iterations per timing window")
     ap.add_argument("--sampling-ratio", type=int, default=None, help="override the config's sampling_ratio (0 = adaptive)")
@@ -489,10 +493,119 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_op(args):
+    """One bench line for a SURVEY 8(f) operation: RoIPool-max fwd+bwd on the config's pyramid / RoIs, greedy NMS or
+    Soft-NMS on `--nms-n` synthetic proposals of one image (log-uniform sizes, 1344 x 800, scores uniform)."""
+    import torch
+    import bench_roofline as roofline
+    from paper_1906_07155_b200 import binding as B
+    from paper_1906_07155_b200 import build as raf_build
+    from paper_1906_07155_b200 import inputs
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(0)
+    raf_build.build()
+    B.lib()
+    stream = torch.cuda.current_stream()
+    peak, peak_src = peaks()
+    sampler = ClockSampler(0)
+
+    def timed(fn, nset):
+        for i in range(max(args.warmup, 3)):
+            fn(i % nset)
+        torch.cuda.synchronize()
+        sampler.start()
+        time.sleep(0.1)
+        ms = []
+        for w in range(args.windows):
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record(stream)
+            for i in range(args.window_iters):
+                fn((w * args.window_iters + i) % nset)
+            a1.record(stream)
+            a1.synchronize()
+            ms.append(a0.elapsed_time(a1) / args.window_iters)
+        return float(np.median(ms)), float(np.min(ms)), sampler.stop()
+
+    if args.op == "pool":
+        cfg = inputs.CONFIGS[args.config]
+        wl = inputs.make_workload(args.config)
+        tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[cfg.dtype]
+        esz = 4 if cfg.dtype == "f32" else 2
+        K, C = cfg.K, cfg.channels
+        PH, PW = cfg.out_size
+        lay = lambda t: t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
+        pyr = sum(int(np.prod(s)) for s in cfg.level_shapes)
+        R = 4
+        feats = [[lay(torch.from_numpy(f).to(tdt).cuda()) for f in wl.feats] for _ in range(R)]
+        rois = torch.from_numpy(wl.rois).cuda()
+        outs = [lay(torch.empty((K, C, PH, PW), dtype=tdt, device="cuda")) for _ in range(R)]
+        args_ = [lay(torch.empty((K, C, PH, PW), dtype=torch.int32, device="cuda")) for _ in range(R)]
+        gouts = [lay(torch.from_numpy(wl.grad_out).to(tdt).cuda()) for _ in range(R)]
+        grads = [[lay(torch.empty(s, dtype=torch.float32, device="cuda")) for s in cfg.level_shapes] for _ in range(R)]
+
+        def step(j):
+            B.roi_pool_fpn_forward(feats[j], cfg.scales, rois, outs[j], args_[j], cfg.finest_scale, stream)
+            B.roi_pool_fpn_backward(grads[j], cfg.scales, gouts[j], args_[j], rois, cfg.finest_scale, 0, stream)
+        ms, ms_min, clocks = timed(step, R)
+        fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, 2, True, cfg.finest_scale)
+        by = fp["union_px"] * C * esz + K * C * PH * PW * (esz + 4) + K * C * PH * PW * (esz + 4) + pyr * 4 * 2
+        ach = by / (ms * 1e-3) / 1e9
+        line = {"metric": "RoIPool-max fwd+bwd RoIs/sec (C=256, 7x7, FPN)", "value": K / (ms * 1e-3), "unit": UNIT,
+                "n_gpus": 1, "steps": args.windows * args.window_iters, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+                "ms_per_step_min": ms_min, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": cfg.dtype, "data": "synthetic",
+                "config": {"workload": f"RoIPool-max on BASELINE.json configs[{args.config - 1}] shapes: {cfg.name}", "K": K, "C": C,
+                           "layout": "cl", "l2_protocol": f"inputs rotate over {R} independent copies"},
+                "roofline": {"bound": "hbm", "kernel": "pool fwd + zero-fill + bwd", "achieved": ach, "peak": peak, "unit": "GB/s",
+                             "frac": ach / peak, "frac_nominal_8000": ach / 8000.0, "traffic": None, "algorithmic_bytes": int(by),
+                             "peak_source": peak_src,
+                             "note": "bytes = touched-pixel union (the RoIAlign union of the same RoIs as a stand-in: RoIPool "
+                                     "windows differ by at most a pixel per side) + out + argmax written + grad_out + argmax "
+                                     "read + gradient pyramid zero-filled and written"},
+                "clocks": clocks, "gpu_launches": args.windows * args.window_iters * (2 + len(cfg.level_shapes))}
+    else:
+        n = args.nms_n
+        rng = np.random.default_rng(190607155 + 77)
+        side = np.exp(rng.uniform(np.log(16), np.log(800), n))
+        asp = np.exp(rng.uniform(np.log(0.5), np.log(2), n))
+        w, h = side * np.sqrt(asp), side / np.sqrt(asp)
+        cx, cy = rng.uniform(0, 1344, n), rng.uniform(0, 800, n)
+        boxes = torch.from_numpy(np.stack([cx - w / 2, cy - h / 2, cx + w / 2, cy + h / 2], 1).astype(np.float32)).cuda()
+        scores = torch.from_numpy(rng.uniform(0, 1, n).astype(np.float32)).cuda()
+        keep = torch.empty(n, dtype=torch.int32, device="cuda")
+        ns = torch.empty(n, dtype=torch.float32, device="cuda")
+        nk = torch.empty(1, dtype=torch.int32, device="cuda")
+        ws = torch.empty(B.roi_nms_workspace_bytes(n), dtype=torch.uint8, device="cuda")
+        if args.op == "nms":
+            fn = lambda j: B.roi_nms(boxes, scores, 0.7, keep, nk, ws, stream)
+            name, launches = f"greedy NMS boxes/sec (n={n} proposals, IoU 0.7)", 3
+        else:
+            fn = lambda j: B.roi_soft_nms(boxes, scores, 0.3, 0.5, 0.05, B.RAF_SOFT_LINEAR, keep, ns, nk, stream)
+            name, launches = f"Soft-NMS (linear) boxes/sec (n={n} proposals)", 1
+        ms, ms_min, clocks = timed(fn, 1)
+        kept = int(nk.item())
+        # ALU bound: the n(n-1)/2 IoU evaluations (about 20 fp32 operations each incl. one IEEE division ~ 10)
+        flops = n * (n - 1) / 2 * 30
+        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        line = {"metric": name, "value": n / (ms * 1e-3), "unit": "boxes/s", "n_gpus": 1,
+                "steps": args.windows * args.window_iters, "warmup": max(args.warmup, 3), "ms_per_step": ms, "ms_per_step_min": ms_min,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": f"{n} boxes of one 1344x800 image, side log-uniform 16-800 px, aspect 0.5-2, scores U(0,1); kept {kept}"},
+                "roofline": {"bound": "alu", "kernel": "nms_mask_kernel" if args.op == "nms" else "soft_nms_kernel",
+                             "achieved": flops / (ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
+                             "frac": flops / (ms * 1e-3) / 1e12 / alu_peak, "traffic": None,
+                             "note": "peak = 148 SMs x 128 fp32 lanes x 2 x 1.965 GHz; the op is latency bound (sequential "
+                                     "scan over kept boxes), the fraction is reported for completeness"},
+                "clocks": clocks, "gpu_launches": args.windows * args.window_iters * launches}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.op != "align":
+        run_op(args)
     else:
         run_ours(args)
 

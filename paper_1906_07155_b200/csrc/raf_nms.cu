@@ -14,7 +14,7 @@
 //   nms_mask_kernel   64 x 64 tiles of the upper triangle: one 64-bit word per (box, tile of later boxes)
 //   nms_scan_kernel   one CTA walks the tiles in order: a single thread resolves the 64 boxes of a tile
 //                     against each other from the diagonal words, then all threads OR the rows of the kept
-//                     boxes into the `removed` bitmap of the later tiles
+//                     boxes into the `removed` bitmap of the later tiles (one (box, word) pair per thread)
 // Soft-NMS is inherently sequential in the emitted box: one CTA keeps the current scores in shared memory
 // and does an arg-max reduction + a decay sweep per emitted box.
 #include "raf_device.cuh"
@@ -108,40 +108,44 @@ nms_scan_kernel(const unsigned long long* __restrict__ mask, const int32_t* __re
                 int32_t* __restrict__ keep, int32_t* __restrict__ num_keep) {
   extern __shared__ unsigned long long s_removed[];   // [nwords]
   __shared__ unsigned long long s_diag[kNmsTile];
-  __shared__ unsigned long long s_kept;
-  __shared__ int s_nk;
+  __shared__ int s_ord[kNmsTile], s_out[kNmsTile], s_bit[kNmsTile];
+  __shared__ int s_nk, s_add;
   for (int w = threadIdx.x; w < nwords; w += blockDim.x) s_removed[w] = 0;
   if (threadIdx.x == 0) s_nk = 0;
   __syncthreads();
   for (int tb = 0; tb < nwords; ++tb) {
     const int m = min(kNmsTile, n - tb * kNmsTile);
-    if (threadIdx.x < m) s_diag[threadIdx.x] = mask[(size_t)(tb * kNmsTile + threadIdx.x) * nwords + tb];
+    if (threadIdx.x < m) {
+      s_diag[threadIdx.x] = mask[(size_t)(tb * kNmsTile + threadIdx.x) * nwords + tb];
+      s_ord[threadIdx.x] = order[tb * kNmsTile + threadIdx.x];
+    }
     __syncthreads();
-    if (threadIdx.x == 0) {   // the 64 boxes of the tile against each other, in order
+    if (threadIdx.x == 0) {   // the 64 boxes of the tile against each other, in order (shared memory only)
       unsigned long long rem = s_removed[tb], kept = 0;
-      int nk = s_nk;
+      int add = 0;
       for (int b = 0; b < m; ++b)
         if (!((rem >> b) & 1ull)) {
           kept |= 1ull << b;
           rem |= s_diag[b];
-          keep[nk++] = order[tb * kNmsTile + b];
+          s_bit[add] = b;
+          s_out[add++] = s_ord[b];
         }
-      s_kept = kept;
-      s_nk = nk;
+      s_add = add;
     }
     __syncthreads();
-    const unsigned long long kept = s_kept;
-    for (int w = tb + 1 + threadIdx.x; w < nwords; w += blockDim.x) {   // rows of the kept boxes -> later tiles
-      unsigned long long acc = 0, kk = kept;
-      while (kk) {
-        const int b = __ffsll((long long)kk) - 1;
-        kk &= kk - 1;
-        acc |= mask[(size_t)(tb * kNmsTile + b) * nwords + w];
-      }
-      s_removed[w] |= acc;
+    if (threadIdx.x < s_add) keep[s_nk + threadIdx.x] = s_out[threadIdx.x];
+    // rows of the kept boxes -> later tiles: one (kept box, word) pair per thread and step, so that all the
+    // loads of a tile are independent (a per-word loop over the kept boxes is a chain of L2 round trips)
+    const int nrem = nwords - tb - 1, npair = s_add * nrem;
+    for (int e = threadIdx.x; e < npair; e += blockDim.x) {
+      const int q = e / nrem, w = tb + 1 + (e - q * nrem);
+      const unsigned long long v = mask[(size_t)(tb * kNmsTile + s_bit[q]) * nwords + w];
+      if (v) atomicOr(&s_removed[w], v);
     }
     __syncthreads();
+    if (threadIdx.x == 0) s_nk += s_add;
   }
+  __syncthreads();
   if (threadIdx.x == 0) *num_keep = s_nk;
 }
 

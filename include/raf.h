@@ -9,7 +9,8 @@
  *
  * General conventions
  *  - Every pointer is a DEVICE pointer unless the parameter comment says HOST.
- *  - The caller owns every buffer, including the workspace.  The library keeps no global state,
+ *  - The caller owns every buffer, including the workspace.  The library keeps no state between calls
+ *    (the one process-wide variable is the monotonic launch counter behind roi_align_fpn_launch_count),
  *    never allocates, never synchronises, never copies device->host (the *_host entry points below
  *    are the stated exception: they copy between the caller's host buffers and the caller's
  *    device arena).  All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the
@@ -37,9 +38,9 @@ typedef enum {
   RAF_ERR_SHAPE = -2,       /* L not in [1,8], K < 0, out_h/out_w not in [1,32], sampling_ratio < 0
                                or > 16, n/c mismatch across levels, non-positive dimension        */
   RAF_ERR_DTYPE = -3,       /* unknown raf_dtype                                                  */
-  RAF_ERR_STRIDE = -4,      /* zero / negative stride, or a stride layout that aliases            */
+  RAF_ERR_STRIDE = -4,      /* zero / negative stride (overlapping strides are the caller's to avoid) */
   RAF_ERR_UNSUPPORTED = -5, /* valid request this version does not implement                      */
-  RAF_ERR_WORKSPACE = -6,   /* ws_bytes smaller than roi_align_fpn_workspace_bytes()              */
+  RAF_ERR_WORKSPACE = -6,   /* ws_bytes smaller than the *_workspace_bytes() query, or ws not 256-aligned */
   RAF_ERR_CUDA = -7         /* a CUDA runtime call / launch failed                                */
 } raf_status;
 
@@ -61,12 +62,14 @@ enum {
                              sampling_ratio > 0, L*N <= 1500)                                       */
   RAF_ATOMIC = 4,         /* force the atomic scatter variant (zero-fill + red.global.add.v4.f32)  */
   RAF_REUSE_PREP = 8      /* the workspace still holds what roi_align_fpn_forward wrote into it when
-                             called with the SAME rois (contents and K), level shapes and scales,
-                             out_h/out_w, sampling_ratio, aligned, finest_scale and workspace pointer:
-                             the backward then skips its own RoI bucketing / tap-table launch.  The
-                             forward always leaves the workspace in that state when it returns RAF_OK;
-                             with different arguments the result is undefined (but memory-safe only
-                             if K and the level shapes match).                                       */
+                             called with the SAME rois pointer and K, level shapes and scales, out_h/out_w,
+                             sampling_ratio, aligned, finest_scale: the backward then skips its own RoI
+                             bucketing / tap-table launch.  The forward leaves the workspace in that state
+                             when it returns RAF_OK (unless RAF_NO_PREP).  The tables carry a fingerprint
+                             of those arguments; on a mismatch (other RoI tensor, other geometry, a
+                             workspace never written) the pull kernel computes nothing from them and fills
+                             the WHOLE gradient pyramid with NaN.  Changing the contents of the rois
+                             buffer in place between the two calls is not detected.                     */
 };
 /* Forward flags (roi_align_fpn_forward_ex). */
 enum {
@@ -98,7 +101,7 @@ int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, i
  *   sampling_ratio  > 0: fixed grid; 0: adaptive gh = ceil(roi_h/out_h), gw = ceil(roi_w/out_w)
  *   aligned      != 0: half-pixel shift, no minimum box size; 0: legacy (no shift, size >= 1)
  *   ws           written: RoI buckets and tap tables that a following roi_align_fpn_backward on the
- *                same arguments may reuse (RAF_REUSE_PREP)                                          */
+ *                same arguments may reuse (RAF_REUSE_PREP); 256-byte aligned                        */
 int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
                           int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
                           void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,

@@ -397,7 +397,9 @@ int roi_align_fpn_forward_host(const raf_level* feats_host, int L, raf_dtype dty
   int rc = check_levels(feats_host, L);
   if (rc) return rc;
   if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
-  if (K < 0 || out_h < 1 || out_w < 1) return RAF_ERR_SHAPE;
+  rc = check_common(rois_host, K, out_h, out_w, sampling_ratio);   // everything host-detectable before the first copy
+  if (rc) return rc;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
   if (!out_strides || !arena || (K > 0 && (!rois_host || !out_host))) return RAF_ERR_NULL;
   if (arena_bytes < roi_align_fpn_host_arena_bytes(feats_host, L, dtype, K, out_h, out_w, sampling_ratio, 0))
     return RAF_ERR_WORKSPACE;
@@ -435,7 +437,11 @@ int roi_align_fpn_backward_host(const raf_level* grad_feats_host, int L, raf_dty
   int rc = check_levels(grad_feats_host, L);
   if (rc) return rc;
   if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
-  if (K < 0 || out_h < 1 || out_w < 1) return RAF_ERR_SHAPE;
+  rc = check_common(rois_host, K, out_h, out_w, sampling_ratio);   // everything host-detectable before the first copy
+  if (rc) return rc;
+  if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP)) return RAF_ERR_UNSUPPORTED;
+  if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
   if (!gout_strides || !arena || (K > 0 && (!rois_host || !grad_out_host))) return RAF_ERR_NULL;
   if (arena_bytes < roi_align_fpn_host_arena_bytes(grad_feats_host, L, gout_dtype, K, out_h, out_w, sampling_ratio, flags))
     return RAF_ERR_WORKSPACE;

@@ -121,14 +121,14 @@ constexpr int kNC = RAF_PULL_NC;   // candidates per build/consume pass
 constexpr int kMaxTapChunks = 4;   // <= 128 taps per axis (eligibility checked on the host)
 constexpr uint32_t kOffMask = 0x00ffffffu;
 
-// Up to two entries of a (candidate, row) or (candidate, column): element offset into grad_out
-// (bin * stride, premultiplied, 24 bits) and weight; the total entry count sits in m0's top byte.
-// More than two entries (bins narrower than half a pixel) are served from the ballot masks.
+// Up to three entries of a (candidate, row) or (candidate, column): the bins with a tap on one pixel row /
+// column are consecutive, so the entry is the element offset of the FIRST bin into grad_out (bin * stride,
+// premultiplied, 24 bits), the weights of the first three bins, and the total entry count in m0's top
+// byte (255 also when the bins turn out not to be consecutive).  More than three entries (bins narrower
+// than about two thirds of a pixel) are served from the ballot masks.
 struct __align__(16) PullInfo {
   uint32_t m0;   // off0 | count << 24
-  float w0;
-  uint32_t off1;
-  float w1;
+  float w0, w1, w2;
 };
 
 // One contribution to a pixel: element offset into grad_out (k*gs_k + ph*gs_h + pw*gs_w) and the
@@ -138,7 +138,10 @@ struct PullPair {
   float w;
 };
 
-template <typename T, bool kFull>
+// kThree: also serve rows / columns with THREE consecutive bins from the entries (outputs finer than the
+// pixel grid, e.g. 14 x 14 mask-head bins: config 4 backward 97.6 -> 90.9 us; on 7 x 7 outputs the extra
+// code in the hit loop costs more than it saves: 87.7 -> 93.0 us, so it is off there).
+template <typename T, bool kFull, bool kThree>
 __global__ void __launch_bounds__(kPullThreads, RAF_PULL_MINB)
 bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gout, int gs_k,
                 int gs_h, int gs_w, const uint32_t* __restrict__ hdr, const int32_t* __restrict__ bperm,
@@ -234,7 +237,7 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
         const int k = s_k[p0 + c];
         const PullTap* ty = taps + (int64_t)k * (nty + ntx);
         const PullTap* tx = ty + nty;
-        int cnt = 0, e0 = -1, e1 = -1;   // lanes 0..7: row `lane`; lanes 8..15: column `lane - 8`
+        int cnt = 0, e0 = -1, e1 = -1, e2 = -1;   // lanes 0..7: row `lane`; lanes 8..15: column `lane - 8`
         for (int q = 0; q < nq; ++q) {
           const int t = q * 32 + lane;
           const int rely = (t < nty) ? (int)(__ldg(&ty[t].pb) & kPixMask) - y0 : -1;
@@ -251,23 +254,31 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
             s_mask[(c * 16 + lane) * nq + q] = mine;
             cnt += __popc(mine);
             if (e0 < 0 && mine) { e0 = q * 32 + __ffs(mine) - 1; mine &= mine - 1; }
-            if (e1 < 0 && mine) e1 = q * 32 + __ffs(mine) - 1;
+            if (e1 < 0 && mine) { e1 = q * 32 + __ffs(mine) - 1; mine &= mine - 1; }
+            if (kThree && e2 < 0 && mine) e2 = q * 32 + __ffs(mine) - 1;
           }
         }
         if (lane < 16) {
           const PullTap* tb = lane < 8 ? ty : tx;
           const uint32_t stride = (uint32_t)(lane < 8 ? gs_h : gs_w);
           PullInfo inf;
-          inf.m0 = 0; inf.w0 = 0.0f; inf.off1 = 0; inf.w1 = 0.0f;
+          inf.m0 = 0; inf.w0 = 0.0f; inf.w1 = 0.0f; inf.w2 = 0.0f;
           if (e0 >= 0) {
             const PullTap e = tb[e0];
-            inf.m0 = ((e.pb >> 24) * stride) | ((uint32_t)min(cnt, 255) << 24);
+            const uint32_t bin0 = e.pb >> 24;
+            int c8 = min(cnt, 255);
             inf.w0 = e.w;
-          }
-          if (e1 >= 0) {
-            const PullTap e = tb[e1];
-            inf.off1 = (e.pb >> 24) * stride;
-            inf.w1 = e.w;
+            if (e1 >= 0) {
+              const PullTap f = tb[e1];
+              inf.w1 = f.w;
+              if ((f.pb >> 24) != bin0 + 1) c8 = 255;   // not consecutive (degenerate box): walk the masks
+            }
+            if (e2 >= 0) {
+              const PullTap f = tb[e2];
+              inf.w2 = f.w;
+              if ((f.pb >> 24) != bin0 + 2) c8 = 255;
+            }
+            inf.m0 = (bin0 * stride) | ((uint32_t)c8 << 24);
           }
           s_info[c][lane] = inf;
         }
@@ -278,8 +289,8 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
         for (int p = lane; p < 8 * npy; p += 32) {
           const PullInfo iy = s_info[c][p >> 3], ix = s_info[c][8 + (p & 7)];
           const uint32_t cy = iy.m0 >> 24, cx = ix.m0 >> 24;
-          const int oy0 = goff + (int)(iy.m0 & kOffMask), oy1 = goff + (int)iy.off1;
-          const int ox0 = (int)(ix.m0 & kOffMask), ox1 = (int)ix.off1;
+          const int oy0 = goff + (int)(iy.m0 & kOffMask), oy1 = oy0 + gs_h;
+          const int ox0 = (int)(ix.m0 & kOffMask), ox1 = ox0 + gs_w;
           uint4 e01, e23;   // order: (y0,x0) (y0,x1) (y1,x0) (y1,x1), absent ones skipped
           e01.x = (uint32_t)(oy0 + ox0); e01.y = __float_as_uint(iy.w0 * ix.w0);
           if (cx >= 2) {
@@ -292,7 +303,8 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
           e23.z = (uint32_t)(oy1 + ox1); e23.w = __float_as_uint(iy.w1 * ix.w1);
           *reinterpret_cast<uint4*>(&s_pair[p][4 * c]) = e01;
           *reinterpret_cast<uint4*>(&s_pair[p][4 * c + 2]) = e23;
-          s_pc[p][c] = (cy == 0 || cx == 0) ? 0 : ((cy > 2 || cx > 2) ? 255 : (unsigned char)(cy * cx));
+          // pair count; 254: up to 3 x 3 consecutive bins, taken from the two entries; 255: walk the masks
+          s_pc[p][c] = (cy == 0 || cx == 0) ? 0 : ((cy > (kThree ? 3 : 2) || cx > (kThree ? 3 : 2)) ? 255 : ((cy > 2 || cx > 2) ? 254 : (unsigned char)(cy * cx)));
         }
       }
       __syncthreads();
@@ -317,7 +329,20 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
           const int c = __ffs(mm) - 1;
           mm &= mm - 1;
           const unsigned np = __shfl_sync(0xffffffffu, pcv, c);
-          if (np != 255u) {
+          if (kThree && np == 254u) {   // three consecutive bins on the row and / or the column: straight from the entries
+            const PullInfo iy = s_info[c][i], ix = s_info[c][8 + j];
+            const int cy = (int)(iy.m0 >> 24), cx = (int)(ix.m0 >> 24);
+            const T* q0 = goutA + s_goff[c] + (int)(iy.m0 & kOffMask) + (int)(ix.m0 & kOffMask);
+            for (int ai = 0; ai < cy; ++ai) {
+              const float wy = ai == 0 ? iy.w0 : (ai == 1 ? iy.w1 : iy.w2);
+              const T* qy = q0 + ai * gs_h;
+              for (int bi = 0; bi < cx; ++bi) {
+                const float w = wy * (bi == 0 ? ix.w0 : (bi == 1 ? ix.w1 : ix.w2));
+                const T* q = qy + bi * gs_w;
+                fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+              }
+            }
+          } else if (np != 255u) {
             const PullPair* sp = &s_pair[p][4 * c];
             const uint4 e01 = *reinterpret_cast<const uint4*>(sp);
             {
@@ -448,14 +473,14 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
   const int rc = pull_plan(lv, a, gs, &pl);
   if (rc) return rc;
   const T* g = reinterpret_cast<const T*>(gout);
-  if (lv.c % 256 == 0)
-    bwd_pull_kernel<T, true><<<pl.grid, kPullThreads, pl.smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], prep.hdr,
-                                                                         prep.bperm, prep.boff, prep.bwin, prep.taps, pl.t,
-                                                                         accumulate, prep.fp);
-  else
-    bwd_pull_kernel<T, false><<<pl.grid, kPullThreads, pl.smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], prep.hdr,
-                                                                          prep.bperm, prep.boff, prep.bwin, prep.taps, pl.t,
-                                                                          accumulate, prep.fp);
+  const bool three = a.PH > 8 || a.PW > 8;
+#define RAF_LAUNCH_PULL(FULL, THREE)                                                                                      \
+  bwd_pull_kernel<T, FULL, THREE><<<pl.grid, kPullThreads, pl.smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], \
+                                                                               prep.hdr, prep.bperm, prep.boff, prep.bwin, \
+                                                                               prep.taps, pl.t, accumulate, prep.fp)
+  if (lv.c % 256 == 0) { if (three) RAF_LAUNCH_PULL(true, true); else RAF_LAUNCH_PULL(true, false); }
+  else { if (three) RAF_LAUNCH_PULL(false, true); else RAF_LAUNCH_PULL(false, false); }
+#undef RAF_LAUNCH_PULL
   count_launch();
   return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;
 }

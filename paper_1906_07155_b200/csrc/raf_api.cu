@@ -2,6 +2,7 @@
 // classification and kernel dispatch.  No allocation, no synchronisation, no device->host copy
 // (except the documented *_host entry points, which copy between caller-owned buffers).
 #include <atomic>
+#include <cstdlib>
 #include <cstring>
 
 #include "raf_device.cuh"
@@ -88,9 +89,9 @@ using namespace raf;
 
 extern "C" {
 
-// Workspace carve-up (pull backward): [hdr 256 B][bperm K int32][boff kBoffInts int32][bwin K int4][taps].
+// Workspace carve-up (pull backward): [hdr 256 B][bperm K int32][boff kBoffInts int32][bwin K int4][bgeo K float4][taps].
 struct WsLayout {
-  size_t hdr, bperm, boff, bwin, taps, total;
+  size_t hdr, bperm, boff, bwin, bgeo, taps, total;
 };
 static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
   const size_t k = K > 0 ? (size_t)K : 0;
@@ -100,7 +101,8 @@ static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
   w.bperm = 256;
   w.boff = w.bperm + align256(4 * k);
   w.bwin = w.boff + align256(4 * (size_t)kBoffInts);
-  w.taps = w.bwin + align256(16 * k);
+  w.bgeo = w.bwin + align256(16 * k);
+  w.taps = w.bgeo + align256(16 * k);
   w.total = w.taps + align256(k * (size_t)(out_h + out_w) * 2 * g * sizeof(PullTap)) + 256;
   return w;
 }
@@ -129,7 +131,7 @@ static PrepFingerprint prep_fingerprint(const raf_level* lv, int L, const float*
     fnv(h, &lv[l].spatial_scale, sizeof(float));
   }
   PrepFingerprint f;
-  f.v[0] = 0x52414631u;   // "RAF1": table format
+  f.v[0] = 0x52414632u;   // "RAF2": table format
   f.v[1] = (uint32_t)K;
   f.v[2] = (uint32_t)out_h | ((uint32_t)out_w << 8) | ((uint32_t)sampling_ratio << 16) | ((uint32_t)(aligned ? 1 : 0) << 24) |
            ((uint32_t)L << 25);
@@ -150,6 +152,7 @@ static PullPrepOut prep_out(void* ws, int K, int out_h, int out_w, int sampling_
   po.bperm = reinterpret_cast<int32_t*>(base + w.bperm);
   po.boff = reinterpret_cast<int32_t*>(base + w.boff);
   po.bwin = reinterpret_cast<int4*>(base + w.bwin);
+  po.bgeo = reinterpret_cast<float4*>(base + w.bgeo);
   po.taps = reinterpret_cast<PullTap*>(base + w.taps);
   po.fp = fp;
   return po;
@@ -248,6 +251,17 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (pull_ok && !(flags & RAF_ATOMIC)) {
     const PullPrepOut po = prep_out(ws, K, out_h, out_w, sampling_ratio, prep_fingerprint(grad_feats, L, rois, K, out_h, out_w, sampling_ratio, aligned,
                                                            finest_scale));
+    bool use_strip = strip_eligible(p, gout_dtype, a, gout_strides) == RAF_OK;
+#ifdef RAF_EXPERIMENT
+    if (const char* e = getenv("RAF_BWD_OLD")) use_strip = use_strip && atoi(e) == 0;
+#endif
+    if (use_strip) {
+      if (!(flags & RAF_REUSE_PREP) || K == 0) {
+        rc = launch_pull_prep(p, a, po, st);
+        if (rc) return rc;
+      }
+      return launch_backward_strip(p, gout_dtype, a, grad_out, gout_strides, po, (flags & RAF_ACCUMULATE) ? 1 : 0, st);
+    }
     rc = pull_eligible(p, gout_dtype, a, grad_out, gout_strides);
     if (rc == RAF_OK) {
       if (!(flags & RAF_REUSE_PREP) || K == 0) {   // else: written by roi_align_fpn_forward on the same arguments

@@ -22,6 +22,7 @@ struct PullPrepOut {
   int32_t* bperm;   // [K]
   int32_t* boff;    // [L*N + 1]
   int4* bwin;       // [K]
+  float4* bgeo;     // [K] {sy, bh, sx, bw} of every kept RoI on its level, bperm order (strip backward)
   PullTap* taps;    // [K][PH + PW][2g]
   int nblocks;      // 1 + ceil(K * (PH + PW) / block size); 0: no prep work in this launch
   PrepFingerprint fp;
@@ -216,6 +217,7 @@ __device__ __forceinline__ void pull_prep_block(const LevelsParam& lv, const Roi
         axis_window(geo.sx, geo.bw, a.PW, a.sampling_ratio, lv.w[level], w.z, w.w);
         if (w.x > w.y || w.z > w.w) w = make_int4(0x7fffffff, -1, 0x7fffffff, -1);
         bwin[p] = w;
+        if (o.bgeo) o.bgeo[p] = make_float4(geo.sy, geo.bh, geo.sx, geo.bw);
       }
     }
     if (key >= 0 && lane == __ffs(peers) - 1) mine[key] = base + __popc(peers);

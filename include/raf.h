@@ -71,6 +71,16 @@ enum {
                              the WHOLE gradient pyramid with NaN.  Changing the contents of the rois
                              buffer in place between the two calls is not detected.                     */
 };
+/* The deterministic pull backward has two kernels with the same contract and the same prep tables: the
+ * TILE kernel (a CTA owns 8 x 8 pixels, one pixel per warp at a time) and the STRIP kernel (a warp owns
+ * a tile and walks it in 8-pixel row strips, loading every grad_out vector once per strip; no limit on
+ * out_h, out_w <= 32 or on the sampling grid).  The library picks per call (strip for large batches of
+ * 7 x 7-like outputs, tile otherwise); these two flags force one of them (RAF_ERR_UNSUPPORTED if that
+ * kernel does not take the arguments; both together are refused). */
+enum {
+  RAF_PULL_STRIP = 32,
+  RAF_PULL_TILE = 64
+};
 /* Forward flags (roi_align_fpn_forward_ex). */
 enum {
   RAF_NO_PREP = 16        /* forward only (inference): do not write the backward's prep tables; the
@@ -118,7 +128,7 @@ int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, con
  *                shapes as the features.  Overwritten (every element written: zero or sum) unless
  *                RAF_ACCUMULATE.
  *   grad_out     DEVICE, dtype = gout_dtype, logical [K,C,out_h,out_w] through gout_strides (HOST)
- *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP                   */
+ *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE */
 int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
                            const void* grad_out, const int64_t* gout_strides, const float* rois,
                            int K, int out_h, int out_w, int sampling_ratio, int aligned,

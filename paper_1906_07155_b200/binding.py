@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(HERE, "libraf.so")
 
 RAF_F32, RAF_F16, RAF_BF16 = 0, 1, 2
 RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC, RAF_REUSE_PREP, RAF_NO_PREP = 1, 2, 4, 8, 16
+RAF_PULL_STRIP, RAF_PULL_TILE = 32, 64
 RAF_SOFT_LINEAR, RAF_SOFT_GAUSSIAN = 1, 2
 _DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_BF16}
 

@@ -61,8 +61,9 @@ static bool levels_vectorizable(const raf_level* lv, int L, int vec, size_t elem
   return true;
 }
 
-static bool tensor_vectorizable(const void* p, const int64_t* s, int vec, size_t elem) {
-  return s[1] == 1 && s[0] % vec == 0 && s[2] % vec == 0 && s[3] % vec == 0 &&
+// (the stride of an extent-1 dimension is never used: frameworks report arbitrary values there)
+static bool tensor_vectorizable(const void* p, const int64_t* s, int vec, size_t elem, int K, int PH, int PW) {
+  return s[1] == 1 && (K <= 1 || s[0] % vec == 0) && (PH <= 1 || s[2] % vec == 0) && (PW <= 1 || s[3] % vec == 0) &&
          ((uintptr_t)p) % (vec * elem) == 0;
 }
 
@@ -211,7 +212,7 @@ int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, con
   const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
   const int vec = (int)(16 / esize(dtype));
   const bool cl = levels_vectorizable(feats, L, vec, esize(dtype)) &&
-                  tensor_vectorizable(out, out_strides, vec, esize(dtype));
+                  tensor_vectorizable(out, out_strides, vec, esize(dtype), K, out_h, out_w);
   // the workspace receives the pull backward's prep tables (consumed by RAF_REUSE_PREP)
   PullPrepOut po{};
   const bool with_prep = want_prep && prep_possible(feats, L, sampling_ratio);
@@ -230,8 +231,10 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (rc) return rc;
   if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
-  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP)) return RAF_ERR_UNSUPPORTED;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE)) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
+  if ((flags & RAF_PULL_STRIP) && (flags & (RAF_PULL_TILE | RAF_ATOMIC))) return RAF_ERR_UNSUPPORTED;
+  if ((flags & RAF_PULL_TILE) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
   if (!gout_strides) return RAF_ERR_NULL;
   for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
   if (K > 0 && !grad_out) return RAF_ERR_NULL;
@@ -244,17 +247,26 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   fill_param(grad_feats, L, &p);
   const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
   const bool cl = levels_vectorizable(grad_feats, L, 4, 4) &&
-                  (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype)));
+                  (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype), K, out_h, out_w));
 
   // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
   const bool pull_ok = cl && prep_possible(grad_feats, L, sampling_ratio);
   if (pull_ok && !(flags & RAF_ATOMIC)) {
     const PullPrepOut po = prep_out(ws, K, out_h, out_w, sampling_ratio, prep_fingerprint(grad_feats, L, rois, K, out_h, out_w, sampling_ratio, aligned,
                                                            finest_scale));
-    bool use_strip = strip_eligible(p, gout_dtype, a, gout_strides) == RAF_OK;
-#ifdef RAF_EXPERIMENT
-    if (const char* e = getenv("RAF_BWD_OLD")) use_strip = use_strip && atoi(e) == 0;
-#endif
+    // Two pull kernels (both deterministic, same prep tables): the strip kernel (raf_backward_strip.cu) wins
+    // when there are many warp tiles to overlap and a grad_out vector feeds several pixels (bins at least
+    // about a pixel wide: the usual 7 x 7 box head); the tile-owned kernel (raf_backward_pull.cu) wins on
+    // small batches and on outputs finer than the pixel grid.  The strip kernel also takes what the
+    // first one cannot (more than 128 taps per axis).
+    const bool strip_ok = strip_eligible(p, gout_dtype, a, gout_strides) == RAF_OK;
+    const bool pull_first_ok = pull_eligible(p, gout_dtype, a, grad_out, gout_strides) == RAF_OK;
+    int64_t pixels = 0;
+    for (int l = 0; l < L; ++l) pixels += (int64_t)grad_feats[l].h * grad_feats[l].w;
+    pixels *= grad_feats[0].n;
+    bool use_strip = strip_ok && (!pull_first_ok || (out_h <= 8 && out_w <= 8 && pixels >= 512 * 1024));
+    if (flags & RAF_PULL_STRIP) { if (!strip_ok) return RAF_ERR_UNSUPPORTED; use_strip = true; }
+    if (flags & RAF_PULL_TILE) { if (!pull_first_ok) return RAF_ERR_UNSUPPORTED; use_strip = false; }
     if (use_strip) {
       if (!(flags & RAF_REUSE_PREP) || K == 0) {
         rc = launch_pull_prep(p, a, po, st);
@@ -273,7 +285,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
     }
     if (rc != RAF_ERR_UNSUPPORTED) return rc;
   }
-  if (flags & RAF_DETERMINISTIC) return RAF_ERR_UNSUPPORTED;
+  if (flags & (RAF_DETERMINISTIC | RAF_PULL_STRIP | RAF_PULL_TILE)) return RAF_ERR_UNSUPPORTED;
 
   // ---- atomic variant (K3) -----------------------------------------------------------------------
   if (!(flags & RAF_ACCUMULATE)) {
@@ -454,8 +466,10 @@ int roi_align_fpn_backward_host(const raf_level* grad_feats_host, int L, raf_dty
   rc = check_common(rois_host, K, out_h, out_w, sampling_ratio);   // everything host-detectable before the first copy
   if (rc) return rc;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
-  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP)) return RAF_ERR_UNSUPPORTED;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE)) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
+  if ((flags & RAF_PULL_STRIP) && (flags & (RAF_PULL_TILE | RAF_ATOMIC))) return RAF_ERR_UNSUPPORTED;
+  if ((flags & RAF_PULL_TILE) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
   if (!gout_strides || !arena || (K > 0 && (!rois_host || !grad_out_host))) return RAF_ERR_NULL;
   if (arena_bytes < roi_align_fpn_host_arena_bytes(grad_feats_host, L, gout_dtype, K, out_h, out_w, sampling_ratio, flags))
     return RAF_ERR_WORKSPACE;

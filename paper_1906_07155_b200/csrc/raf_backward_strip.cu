@@ -20,22 +20,31 @@
 //
 // Per warp tile:
 //  (A) scan: the lanes test the conservative pixel windows `bwin` of the tile's (level, image) bucket
-//      against the tile, 128 records per round trip, and keep the first NC RoIs that meet it (bucket
+//      against the tile, 288 records per round trip, and keep the next NC RoIs that meet it (bucket
 //      order = ascending k: fixed summation order); their geometry `bgeo` and grad_out row offset
-//      follow in one more round trip.  A tile that meets more than NC RoIs is processed row by row,
-//      each row taking the bucket in batches of NC with its accumulators kept across batches.
+//      follow in one more round trip.  A tile that meets more than NC RoIs takes the bucket in several
+//      batches; later batches add to what the earlier ones stored (one-row tiles keep their sums in
+//      registers instead).
 //  (B) tables: one lane per (candidate, axis, bin) evaluates the bin's g samples with the canonical
 //      fp32 coordinate arithmetic (raf_device.cuh, bit-identical to the forward) and leaves DENSE
-//      weights in the warp's shared memory: xw[c][pw][8 columns], yw[c][8 rows][ph], plus the column /
-//      row occupancy bits of every bin.  No tap tables in global memory.
-//  (C) the warp flattens what the rows receive into a WORK LIST (one item per (row, candidate, ph, pw)
-//      with a tap on the row and inside the strip: grad_out offset, wy, column weights, column mask)
-//      and consumes it through a ring of cp.async stages: the vectors of the next kRing - 1 items --
-//      across row boundaries -- are in flight while the current one is FMA'd (memory-level
-//      parallelism at no register cost; each lane copies and reads back its own 16 bytes).
+//      weights in the warp's shared memory: xw[c][pw][8 columns], yw[c][8 rows][ph], the ph bits with a
+//      tap on every row and the list of bins with a tap inside the strip.  No tap tables in global memory.
+//  (C) work list: lane c owns candidate c and emits its items -- one per (row, ph, pw) with a tap on the
+//      row and inside the strip: grad_out offset, column mask, wy * xw[8 columns] -- at the positions a
+//      warp prefix sum assigns (row-major, then c, ph, pw).  The warp consumes the list through a ring
+//      of cp.async stages: the vectors of the next kRing - 1 items, across row boundaries, are in flight
+//      while the current one is FMA'd with packed fp32x2 FMAs (memory-level parallelism at no register
+//      cost; each lane copies and reads back its own 16 bytes, so no barrier is needed).
 //  (D) a row is stored when its last item is done (zero where nothing lands; added to the old value
-//      with RAF_ACCUMULATE).
-// Any sampling grid g >= 1 and any out_h / out_w <= 32 take this path.
+//      with RAF_ACCUMULATE or in a later batch).
+// Any sampling grid g >= 1 and any out_h / out_w <= 32 take this path (no tap-count limit).
+//
+// Measured (B200, cold-L2 rotation, profiles/r2_backward.md): config 5 (16 images, 25.8 K warp tiles)
+// 516 -> 455 us against the first generation; on config 2 (2 images, 3.2 K warp tiles = 1.8 waves of
+// 12 resident warps per SM) the fixed ~8 us of dependent round trips per tile is not covered and the
+// first generation stays ahead (89 vs 95 us), as it does for outputs finer than the pixel grid
+// (14 x 14 bins: a vector then feeds only 1-2 pixels, so loading it once per strip buys nothing).
+// raf_api.cu picks per call.
 #include "raf_device.cuh"
 #include "raf_host.h"
 #include "raf_pull_prep.cuh"
@@ -58,7 +67,7 @@ constexpr int kRing = RAF_STRIP_RING;          // cp.async stages per warp
 #define RAF_STRIP_WORK 96
 #endif
 constexpr int kWorkCap = RAF_STRIP_WORK;       // work-list items per flush (>= 32)
-constexpr int kScanRounds = 4;                 // bucket records per lane and round trip
+constexpr int kScanRounds = 9;                 // bucket records per lane and round trip
 
 struct StripLevels {
   float* data[kMaxLevels];
@@ -71,15 +80,6 @@ struct StripLevels {
   int32_t order[kMaxLevels];      // level at schedule position i
   int32_t L, N, C, chunks;
   int32_t total;                  // warp tiles = tiles x N x chunks
-};
-
-// One grad_out vector a strip needs: element offset of gout[k][ph][pw], index of its column weights,
-// the row weight wy (1/count folded in) and the columns of the strip it touches.
-struct __align__(16) StripItem {
-  int goff;
-  int xref;
-  float wy;
-  uint32_t xmask;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -116,9 +116,13 @@ template <> struct StripVec<__nv_bfloat16> {
   }
 };
 
+// acc += w * v on 4 channels with two packed fp32x2 FMAs (sm_100: one issue slot per two FMAs; each half
+// rounds exactly like fmaf).
 __device__ __forceinline__ void strip_fma(float4& acc, float w, const float4& v) {
-  acc.x = fmaf(w, v.x, acc.x); acc.y = fmaf(w, v.y, acc.y);
-  acc.z = fmaf(w, v.z, acc.z); acc.w = fmaf(w, v.w, acc.w);
+  const float2 ww = make_float2(w, w);
+  const float2 lo = __ffma2_rn(ww, make_float2(v.x, v.y), make_float2(acc.x, acc.y));
+  const float2 hi = __ffma2_rn(ww, make_float2(v.z, v.w), make_float2(acc.z, acc.w));
+  acc = make_float4(lo.x, lo.y, hi.x, hi.y);
 }
 
 // Dense weights of one output bin along one axis on the 8 pixels [origin, origin + 8): the bin's g
@@ -145,7 +149,7 @@ __device__ __forceinline__ uint32_t strip_bin_weights(float start, float bsz, in
 // Per-warp shared memory (bytes), in this order: ring | work list | xw | yw | cgeo | xl | yph | cgoff | rowend | cnb.
 __host__ __device__ inline size_t strip_warp_smem(int NC, int PH, int PW, size_t esz) {
   size_t s = (size_t)kRing * 256 * esz;
-  s += sizeof(StripItem) * kWorkCap;
+  s += 40 * (size_t)(kWorkCap + 2);
   s += sizeof(float) * NC * PW * 8;
   s += sizeof(float) * NC * 8 * PH;
   s += 16 * (size_t)NC + 8 * (size_t)NC * PW + 4 * (size_t)NC * 8 + 4 * (size_t)NC + 4 * (kStripMaxRows + 1);
@@ -154,6 +158,7 @@ __host__ __device__ inline size_t strip_warp_smem(int NC, int PH, int PW, size_t
 }
 
 __device__ __forceinline__ int strip_pow2_lanes(int P) { return P <= 8 ? 8 : (P <= 16 ? 16 : 32); }
+
 
 template <typename T, bool kFull>
 __global__ void __launch_bounds__(32 * kStripWarps)
@@ -172,7 +177,9 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
   // ---- this warp's shared memory --------------------------------------------------------------------
   unsigned char* sp = strip_smem + (size_t)warp * strip_warp_smem(NC, PH, PW, sizeof(T));
   unsigned char* ring = sp;                            sp += (size_t)kRing * kStage;
-  StripItem* work = reinterpret_cast<StripItem*>(sp);  sp += sizeof(StripItem) * kWorkCap;
+  float4* work_wa = reinterpret_cast<float4*>(sp);     sp += 16 * (size_t)(kWorkCap + 2);   // wy * xw[columns 0..3] per item
+  float4* work_wb = reinterpret_cast<float4*>(sp);     sp += 16 * (size_t)(kWorkCap + 2);   // wy * xw[columns 4..7]
+  int2* work_hd = reinterpret_cast<int2*>(sp);         sp += 8 * (size_t)(kWorkCap + 2);    // {grad_out offset, column mask}
   float* s_xw = reinterpret_cast<float*>(sp);          sp += sizeof(float) * NC * PW * 8;   // [c][pw][column]
   float* s_yw = reinterpret_cast<float*>(sp);          sp += sizeof(float) * NC * 8 * PH;   // [c][row][ph]
   float4* s_cgeo = reinterpret_cast<float4*>(sp);      sp += 16 * (size_t)NC;               // {sy, bh, sx, bw}
@@ -222,13 +229,13 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
       acc[j][1] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   };
-  auto store_row = [&](int r) {
+  auto store_row = [&](int r, bool add_old) {
     float* gp = gtile + r * sh;
 #pragma unroll
     for (int j = 0; j < kStripCols; ++j) {
       if (j < npx) {
         float4 vA = acc[j][0], vB = acc[j][1];
-        if (accumulate) {
+        if (add_old) {
           if (actA) { const float4 o = *reinterpret_cast<const float4*>(gp); vA.x += o.x; vA.y += o.y; vA.z += o.z; vA.w += o.w; }
           if (actB) { const float4 o = *reinterpret_cast<const float4*>(gp + 128); vB.x += o.x; vB.y += o.y; vB.z += o.z; vB.w += o.w; }
         }
@@ -252,23 +259,22 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
       acc[j][0] = make_float4(qnan, qnan, qnan, qnan);
       acc[j][1] = acc[j][0];
     }
-    accumulate = 0;
-    for (int r = 0; r < npy; ++r) store_row(r);
+    for (int r = 0; r < npy; ++r) store_row(r, false);
     return;
   }
 
   const int P2y = strip_pow2_lanes(PH), P2x = strip_pow2_lanes(PW);
 
-  // Rows [rb, rb + nr) are processed together when the tile meets at most NC RoIs (the usual case: one
-  // scan, one table build, one work list across the rows); otherwise one row at a time.
-  int rstep = npy;
-  for (int rb = 0; rb < npy; rb += rstep) {
-    int nr = min(rstep, npy - rb);
-    int spos = bbeg;
+  // The bucket is taken in batches of NC RoIs (usually one batch: one scan, one table build, one work list
+  // across the rows of the tile).  Later batches add to what the earlier ones stored (tiles of one row
+  // keep their sums in registers instead): the summation order stays fixed.
+  {
+    const int rb = 0, nr = npy;
+    int spos = bbeg, batch = 0;
     zero_acc();
     while (true) {
-      // ---- (A) the next <= NC RoIs of the bucket whose window meets rows [rb, rb + nr) of the tile ----
-      const int ya = y0 + rb, yb = ya + nr - 1;
+      // ---- (A) the next <= NC RoIs of the bucket whose window meets the tile ---------------------------
+      const int ya = y0, yb = y0 + npy - 1;
       int ncand = 0;
       while (spos < bend && ncand < NC) {
         int4 wv[kScanRounds];
@@ -297,10 +303,7 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
       }
       if (spos > bend) spos = bend;
       const bool last = spos >= bend;
-      if (!last && nr > 1) {   // more than NC RoIs meet the tile: row by row from here on
-        rstep = 1; nr = 1; spos = bbeg;
-        continue;
-      }
+      if (ncand == 0 && batch > 0 && npy > 1) break;   // (the bucket ended exactly at a batch boundary)
       __syncwarp();
       for (int c = lane; c < ncand; c += 32) {
         const int i = s_cgoff[c];
@@ -368,18 +371,22 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
           const int total = __shfl_sync(0xffffffffu, incl, 31);
           const int space = kWorkCap - nitems;
           const int start = incl - remc;
-          int nem = min(remc, space - start);
-          StripItem* wp = work + nitems + start;
-          for (int i = 0; i < nem; ++i) {
-            const int ph = __ffs(ym) - 1;
-            const int2 xe = s_xl[lane * PW + e];
-            StripItem it;
-            it.goff = goffc + ph * gs_h + xe.x;
-            it.xref = (int)((uint32_t)xe.y >> 8);
-            it.wy = s_yw[(lane * 8 + r) * PH + ph];
-            it.xmask = (uint32_t)xe.y & 0xffu;
-            wp[i] = it;
-            if (++e == nbl) { e = 0; ym &= ym - 1; }
+          const int nem = min(remc, space - start);
+          if (nem > 0) {
+            const float* ywp = s_yw + (lane * 8 + r) * PH;
+            const int2* xl = s_xl + lane * PW;
+            const int at = nitems + start;
+            for (int i = 0; i < nem; ++i) {
+              const int ph = __ffs(ym) - 1;
+              const int2 xe = xl[e];
+              const float wy = ywp[ph];
+              const float* xw = s_xw + ((uint32_t)xe.y >> 8);
+              const float4 xa = *reinterpret_cast<const float4*>(xw), xb = *reinterpret_cast<const float4*>(xw + 4);
+              work_hd[at + i] = make_int2(goffc + ph * gs_h + xe.x, xe.y & 0xff);
+              work_wa[at + i] = make_float4(wy * xa.x, wy * xa.y, wy * xa.z, wy * xa.w);
+              work_wb[at + i] = make_float4(wy * xb.x, wy * xb.y, wy * xb.z, wy * xb.w);
+              if (++e == nbl) { e = 0; ym &= ym - 1; }
+            }
           }
           if (total > space) { nitems = kWorkCap; break; }   // flush, then go on with this row
           nitems += total;
@@ -389,44 +396,46 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
           e = 0;
         }
         __syncwarp();
-        // consume: item t is FMA'd while items t+1 .. t+kRing-1 are in flight
+        // consume: item t is FMA'd while items t+1 .. t+kRing-1 are in flight; its header and weights
+        // are read one item ahead
 #pragma unroll 1
         for (int t = 0; t < kRing - 1; ++t) {
-          if (t < nitems) prefetch(work[t].goff, t);
+          if (t < nitems) prefetch(work_hd[t].x, t);
           cp_async_commit();
         }
         int t = 0, slot = 0, pslot = kRing - 1;
+        int2 hd = work_hd[0];
+        float4 wa = work_wa[0], wb = work_wb[0];
         for (int rr = rdone; rr <= r && rr < rb + nr; ++rr) {
           const int tend = rr < r ? s_rowend[rr - rb] : nitems;
 #pragma unroll 1
           for (; t < tend; ++t) {
-            if (t + kRing - 1 < nitems) prefetch(work[t + kRing - 1].goff, pslot);
+            if (t + kRing - 1 < nitems) prefetch(work_hd[t + kRing - 1].x, pslot);
             cp_async_commit();
             cp_async_wait<kRing - 1>();
-            const StripItem it = work[t];
             const unsigned char* stage = ring_rd + slot * kStage;
             const float4 vA = SV::read(stage), vB = SV::read(stage + 32 * SV::kBytes);
+            const int2 hd_n = work_hd[t + 1];
+            const float4 wa_n = work_wa[t + 1], wb_n = work_wb[t + 1];
             slot = slot + 1 == kRing ? 0 : slot + 1;
             pslot = pslot + 1 == kRing ? 0 : pslot + 1;
-            if (it.xmask & 0x0fu) {
-              const float4 xw = *reinterpret_cast<const float4*>(s_xw + it.xref);
-              const float w0 = it.wy * xw.x, w1 = it.wy * xw.y, w2 = it.wy * xw.z, w3 = it.wy * xw.w;
-              strip_fma(acc[0][0], w0, vA); strip_fma(acc[0][1], w0, vB);
-              strip_fma(acc[1][0], w1, vA); strip_fma(acc[1][1], w1, vB);
-              strip_fma(acc[2][0], w2, vA); strip_fma(acc[2][1], w2, vB);
-              strip_fma(acc[3][0], w3, vA); strip_fma(acc[3][1], w3, vB);
+            if (hd.y & 0x0f) {
+              strip_fma(acc[0][0], wa.x, vA); strip_fma(acc[0][1], wa.x, vB);
+              strip_fma(acc[1][0], wa.y, vA); strip_fma(acc[1][1], wa.y, vB);
+              strip_fma(acc[2][0], wa.z, vA); strip_fma(acc[2][1], wa.z, vB);
+              strip_fma(acc[3][0], wa.w, vA); strip_fma(acc[3][1], wa.w, vB);
             }
-            if (it.xmask & 0xf0u) {
-              const float4 xw = *reinterpret_cast<const float4*>(s_xw + it.xref + 4);
-              const float w0 = it.wy * xw.x, w1 = it.wy * xw.y, w2 = it.wy * xw.z, w3 = it.wy * xw.w;
-              strip_fma(acc[4][0], w0, vA); strip_fma(acc[4][1], w0, vB);
-              strip_fma(acc[5][0], w1, vA); strip_fma(acc[5][1], w1, vB);
-              strip_fma(acc[6][0], w2, vA); strip_fma(acc[6][1], w2, vB);
-              strip_fma(acc[7][0], w3, vA); strip_fma(acc[7][1], w3, vB);
+            if (hd.y & 0xf0) {
+              strip_fma(acc[4][0], wb.x, vA); strip_fma(acc[4][1], wb.x, vB);
+              strip_fma(acc[5][0], wb.y, vA); strip_fma(acc[5][1], wb.y, vB);
+              strip_fma(acc[6][0], wb.z, vA); strip_fma(acc[6][1], wb.z, vB);
+              strip_fma(acc[7][0], wb.w, vA); strip_fma(acc[7][1], wb.w, vB);
             }
+            hd = hd_n; wa = wa_n; wb = wb_n;
           }
           if (rr < r) {   // every item of row rr (of this batch) is in
-            if (last) { store_row(rr); zero_acc(); }
+            if (npy > 1) { store_row(rr, accumulate || batch > 0); zero_acc(); }
+            else if (last) store_row(rr, accumulate != 0);
             rdone = rr + 1;
           }
         }
@@ -434,6 +443,7 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
         __syncwarp();   // the work list is rewritten by the next flush
       }
       if (last) break;
+      ++batch;
     }
   }
 }
@@ -474,6 +484,9 @@ static int strip_plan(const LevelsParam& lv, const RoiArgs& a, const int64_t* gs
     t.tiles_x[l] = (lv.w[l] + kStripCols - 1) / kStripCols;
     int th = kStripMaxRows;   // dense coarse levels get short tiles: more, shorter warp tiles where the RoIs pile up
     while (th > 1 && (int64_t)((lv.h[l] + th - 1) / th) * t.tiles_x[l] < mintiles) th >>= 1;
+#ifdef RAF_EXPERIMENT
+    if (const char* e = getenv("RAF_TUNE_TH")) { if ((int)strlen(e) > 2 * l) th = e[2 * l] - '0'; }   // e.g. "8,4,2,1"
+#endif
     t.th[l] = th;
     t.start[i] = (int32_t)total;
     total += (int64_t)((lv.h[l] + th - 1) / th) * t.tiles_x[l];

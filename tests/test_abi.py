@@ -108,7 +108,8 @@ def test_backward_argument_errors(lib):
     assert bwd(_levels(), K=-2) == -2
     assert bwd(_levels(), dtype=3) == -3
     assert bwd(_levels(sn=-5)) == -4
-    assert bwd(_levels(), flags=64) == -5                          # RAF_ERR_UNSUPPORTED
+    assert bwd(_levels(), flags=1024) == -5                        # RAF_ERR_UNSUPPORTED (unknown flag)
+    assert bwd(_levels(), flags=32 | 64) == -5                     # RAF_PULL_STRIP with RAF_PULL_TILE
     assert bwd(_levels(), ws_bytes=0) == -6
 
 

@@ -169,7 +169,8 @@ def _bwd_case(wl, gout_dtype, layout, P=None, g=None, aligned=None, flags=0, ini
     return T.assert_backward_close(got, ref, S)
 
 
-VARIANTS = [("cl", 0), ("cl", B.RAF_ATOMIC), ("cl", B.RAF_DETERMINISTIC), ("nchw", 0)]
+VARIANTS = [("cl", 0), ("cl", B.RAF_ATOMIC), ("cl", B.RAF_DETERMINISTIC), ("cl", B.RAF_PULL_STRIP),
+            ("cl", B.RAF_PULL_TILE), ("nchw", 0)]
 
 
 @pytest.mark.parametrize("layout,flags", VARIANTS)
@@ -190,12 +191,17 @@ def test_backward_reduced_configs(index, dtype, kw, layout, flags):
     _bwd_case(inputs.make_workload(index, **kw), dtype, layout, flags=flags)
 
 
-@pytest.mark.parametrize("layout,flags", [("cl", 0), ("cl", B.RAF_ATOMIC), ("nchw", 0)])
+@pytest.mark.parametrize("layout,flags", [("cl", 0), ("cl", B.RAF_ATOMIC), ("cl", B.RAF_PULL_STRIP), ("nchw", 0)])
 @pytest.mark.parametrize("P,g,aligned", [((7, 7), 1, True), ((7, 7), 0, True), ((7, 7), 2, False),
                                          ((5, 9), 3, True), ((14, 14), 2, True), ((7, 7), 0, False),
                                          ((32, 32), 2, True), ((1, 1), 4, True), ((3, 2), 16, False)])
 def test_backward_variants(P, g, aligned, layout, flags):
     wl = inputs.make_workload(5, n_img=2, per_img=24, channels=8)
+    if flags == B.RAF_PULL_STRIP and g == 0:   # the pull kernels need a fixed sampling grid: refused, not downgraded
+        with pytest.raises(B.RafError) as e:
+            _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned, flags=flags)
+        assert e.value.status == -5
+        return
     _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned, flags=flags)
 
 
@@ -215,12 +221,12 @@ def _single_level_case(K, C, H, W, side_lo, side_hi, seed, flags, P=(7, 7), g=2,
     return T.assert_backward_close(got, ref, S)
 
 
-@pytest.mark.parametrize("flags", [0, B.RAF_DETERMINISTIC, B.RAF_ATOMIC])
+@pytest.mark.parametrize("flags", [0, B.RAF_DETERMINISTIC, B.RAF_ATOMIC, B.RAF_PULL_STRIP, B.RAF_PULL_TILE])
 def test_backward_dense_tiles_and_big_buckets(flags):
     _single_level_case(K=700, C=16, H=24, W=40, side_lo=4, side_hi=20, seed=11, flags=flags)
 
 
-@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC])
+@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC, B.RAF_PULL_STRIP])
 @pytest.mark.parametrize("C,dtype", [(8, "f32"), (320, "f32"), (264, "bf16")])
 def test_backward_tiny_boxes_many_entries_per_pixel(flags, C, dtype):
     # boxes of 0.3 .. 3 px: bins narrower than half a pixel -> up to 7 entries per row / column
@@ -228,21 +234,23 @@ def test_backward_tiny_boxes_many_entries_per_pixel(flags, C, dtype):
 
 
 @pytest.mark.parametrize("P,g", [((14, 14), 2), ((9, 20), 3)])
-def test_backward_many_taps_dense(P, g):
-    # more than 32 taps per axis (two / four ballot chunks) on a dense map
-    _single_level_case(K=120, C=12, H=20, W=20, side_lo=2, side_hi=18, seed=13, flags=0, P=P, g=g)
+@pytest.mark.parametrize("flags", [B.RAF_PULL_TILE, B.RAF_PULL_STRIP])
+def test_backward_many_taps_dense(P, g, flags):
+    # more than 32 taps per axis (two / four ballot chunks of the tile kernel) on a dense map
+    _single_level_case(K=120, C=12, H=20, W=20, side_lo=2, side_hi=18, seed=13, flags=flags, P=P, g=g)
 
 
-@pytest.mark.parametrize("flags", [0, B.RAF_DETERMINISTIC])
+@pytest.mark.parametrize("flags", [0, B.RAF_DETERMINISTIC, B.RAF_PULL_STRIP])
 def test_backward_largest_output_and_grid(flags):
     # 32 x 32 bins with a 4 x 4 sampling grid (256 sample taps per axis): the largest output the ABI takes;
     # the strip backward's dense per-bin weights have no tap-count limit, so this is deterministic too
     _single_level_case(K=20, C=8, H=20, W=20, side_lo=2, side_hi=18, seed=14, flags=flags, P=(32, 32), g=4)
 
 
+@pytest.mark.parametrize("variant", [B.RAF_PULL_TILE, B.RAF_PULL_STRIP])
 @pytest.mark.parametrize("layout_fwd", ["cl", "nchw"])
 @pytest.mark.parametrize("dtype", ["f32", "bf16"])
-def test_backward_reuses_prep_written_by_forward(layout_fwd, dtype):
+def test_backward_reuses_prep_written_by_forward(layout_fwd, dtype, variant):
     """RAF_REUSE_PREP: the forward call leaves the RoI buckets / tap tables in the workspace (in the
     leading blocks of its own launch for channels-last, by a separate launch otherwise); the backward
     skips its prep launch.  Result must equal the oracle and the stand-alone backward bit for bit."""
@@ -259,11 +267,11 @@ def test_backward_reuses_prep_written_by_forward(layout_fwd, dtype):
     out = T.empty_layout((K, C, PH, PW), feats[0].dtype, layout_fwd)
     B.roi_align_fpn_forward(feats, cfg.scales, rois, out, 2, True, cfg.finest_scale, ws)
     g1 = [T.empty_layout(s, torch.float32, "cl", fill=float("nan")) for s in cfg.level_shapes]
-    B.roi_align_fpn_backward(g1, cfg.scales, go, rois, 2, True, cfg.finest_scale, B.RAF_REUSE_PREP, ws)
+    B.roi_align_fpn_backward(g1, cfg.scales, go, rois, 2, True, cfg.finest_scale, B.RAF_REUSE_PREP | variant, ws)
     torch.cuda.synchronize()
     ws2 = T.workspace(K, L, PH, PW, 2)
     g2 = [T.empty_layout(s, torch.float32, "cl", fill=float("nan")) for s in cfg.level_shapes]
-    B.roi_align_fpn_backward(g2, cfg.scales, go, rois, 2, True, cfg.finest_scale, 0, ws2)
+    B.roi_align_fpn_backward(g2, cfg.scales, go, rois, 2, True, cfg.finest_scale, variant, ws2)
     torch.cuda.synchronize()
     for a_, b_ in zip(g1, g2):
         assert torch.equal(a_, b_)
@@ -287,11 +295,12 @@ def test_backward_degenerate_and_invalid_rois():
         T.assert_backward_close(got, ref, S)
 
 
-def test_deterministic_backward_is_bit_reproducible():
+@pytest.mark.parametrize("variant", [0, B.RAF_PULL_STRIP, B.RAF_PULL_TILE])
+def test_deterministic_backward_is_bit_reproducible(variant):
     wl = inputs.make_workload(5, n_img=3, per_img=200, channels=64)
     cfg = wl.cfg
     runs = [T.gpu_backward(cfg.level_shapes, cfg.scales, wl.grad_out, wl.rois, 2, True, 56.0, "cl", "bf16",
-                           B.RAF_DETERMINISTIC)[0] for _ in range(3)]
+                           B.RAF_DETERMINISTIC | variant)[0] for _ in range(3)]
     for other in runs[1:]:
         for a, b in zip(runs[0], other):
             assert np.array_equal(a, b)
@@ -310,7 +319,7 @@ def test_backward_accumulate_mode(layout, flags):
     _bwd_case(wl, "f32", layout, flags=flags | B.RAF_ACCUMULATE, init=init)
 
 
-@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC])
+@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC, B.RAF_PULL_STRIP])
 def test_backward_full_size_config2(flags):
     wl = inputs.make_workload(2, with_feats=False)
     cfg = wl.cfg
@@ -381,7 +390,8 @@ def test_backward_full_size_config5_atomic():
         T.assert_backward_close([g[:, sl] for g in got], ref, S)
 
 
-def test_reuse_prep_with_foreign_workspace_is_loud():
+@pytest.mark.parametrize("variant", [B.RAF_PULL_TILE, B.RAF_PULL_STRIP])
+def test_reuse_prep_with_foreign_workspace_is_loud(variant):
     """RAF_REUSE_PREP on a workspace that was NOT written for these arguments (forward on other RoIs, other
     K, other geometry, or never written at all): the pull kernel compares the fingerprint the prep left and
     poisons the whole gradient pyramid with NaN instead of computing from foreign tables."""
@@ -397,7 +407,7 @@ def test_reuse_prep_with_foreign_workspace_is_loud():
 
     def bwd(rois_t, ws, flags, g=2, aligned=True):
         grads = [T.empty_layout(s, torch.float32, "cl", fill=1.0) for s in cfg.level_shapes]
-        B.roi_align_fpn_backward(grads, cfg.scales, go, rois_t, g, aligned, cfg.finest_scale, flags, ws)
+        B.roi_align_fpn_backward(grads, cfg.scales, go, rois_t, g, aligned, cfg.finest_scale, flags | variant, ws)
         torch.cuda.synchronize()
         return grads
 
@@ -542,7 +552,7 @@ def _margins_intact(buf, nbytes, margin=4096):
     (5, "bf16", dict(n_img=2, per_img=100, channels=40), (7, 7)),     # boxes partly outside, partial chunk
     (4, "f16", dict(n_img=1, per_img=60, channels=264), (14, 14)),
 ])
-@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC, B.RAF_REUSE_PREP])
+@pytest.mark.parametrize("flags", [0, B.RAF_ATOMIC, B.RAF_REUSE_PREP, B.RAF_PULL_STRIP, B.RAF_PULL_STRIP | B.RAF_REUSE_PREP])
 def test_no_out_of_bounds_writes(index, dtype, kw, P, flags):
     wl = inputs.make_workload(index, **kw)
     cfg = wl.cfg

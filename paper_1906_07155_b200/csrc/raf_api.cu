@@ -111,7 +111,7 @@ static WsLayout ws_layout(int K, int out_h, int out_w, int sampling_ratio) {
 // The pull backward's prep tables can be built for these arguments (layout-independent part of the
 // pull eligibility; the forward uses the same test before it writes them into the workspace).
 static bool prep_possible(const raf_level* lv, int L, int sampling_ratio) {
-  if (sampling_ratio <= 0 || (int64_t)L * lv[0].n + 1 > kBoffInts) return false;
+  if (sampling_ratio < 0 || (int64_t)L * lv[0].n + 1 > kBoffInts) return false;   // (0 = adaptive: buckets only)
   if (bucket_smem_bytes(L, lv[0].n) > 200 * 1024) return false;
   if ((size_t)(kMaxLevels + 1) * ((size_t)L * lv[0].n + 1) * sizeof(int) > 200 * 1024) return false;
   for (int l = 0; l < L; ++l)   // tap tables keep pixel indices in 24 bits

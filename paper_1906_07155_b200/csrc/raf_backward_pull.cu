@@ -106,9 +106,17 @@ template <typename T> struct Gout8 {
   }
 };
 
+// acc += w * v on 4 channels: two packed fp32x2 FMAs (sm_100; each half rounds exactly like fmaf)
 __device__ __forceinline__ void fma4(float4& acc, float w, const float4& v) {
+#ifndef RAF_NO_FFMA2
+  const float2 ww = make_float2(w, w);
+  const float2 lo = __ffma2_rn(ww, make_float2(v.x, v.y), make_float2(acc.x, acc.y));
+  const float2 hi = __ffma2_rn(ww, make_float2(v.z, v.w), make_float2(acc.z, acc.w));
+  acc = make_float4(lo.x, lo.y, hi.x, hi.y);
+#else
   acc.x = fmaf(w, v.x, acc.x); acc.y = fmaf(w, v.y, acc.y);
   acc.z = fmaf(w, v.z, acc.z); acc.w = fmaf(w, v.w, acc.w);
+#endif
 }
 
 #ifndef RAF_PULL_NC

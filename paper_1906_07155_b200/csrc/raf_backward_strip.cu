@@ -37,7 +37,8 @@
 //      cost; each lane copies and reads back its own 16 bytes, so no barrier is needed).
 //  (D) a row is stored when its last item is done (zero where nothing lands; added to the old value
 //      with RAF_ACCUMULATE or in a later batch).
-// Any sampling grid g >= 1 and any out_h / out_w <= 32 take this path (no tap-count limit).
+// Any sampling grid (fixed g >= 1, or the adaptive per-RoI grid of sampling_ratio == 0) and any
+// out_h / out_w <= 32 take this path (no tap-count limit).
 //
 // Measured (B200, cold-L2 rotation, profiles/r2_backward.md): config 5 (16 images, 25.8 K warp tiles)
 // 516 -> 455 us against the first generation; on config 2 (2 images, 3.2 K warp tiles = 1.8 waves of
@@ -220,7 +221,6 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
   const uint32_t ring_u32 = smem_u32(ring) + lane * SV::kBytes;
   const unsigned char* ring_rd = ring + lane * SV::kBytes;
   const unsigned lt_mask = (1u << lane) - 1u;
-  const float inv_count = 1.0f / (float)(g * g);
 
   auto zero_acc = [&]() {
 #pragma unroll
@@ -320,7 +320,9 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
         uint32_t m = 0;
         if (val) {
           const float4 geo = s_cgeo[c];
-          m = strip_bin_weights(geo.x, geo.y, ph, g, H, inv_count, y0, w);
+          const int gh = sampling_grid(g, geo.y), gw = sampling_grid(g, geo.w);   // (the fixed grid, or per RoI)
+          const int cnt = gh * gw;
+          m = strip_bin_weights(geo.x, geo.y, ph, gh, H, 1.0f / (float)(cnt > 1 ? cnt : 1), y0, w);
 #pragma unroll
           for (int r = 0; r < 8; ++r) s_yw[(c * 8 + r) * PH + ph] = w[r];
         }
@@ -338,7 +340,7 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
         uint32_t m = 0;
         if (val) {
           const float4 geo = s_cgeo[c];
-          m = strip_bin_weights(geo.z, geo.w, pw, g, W, 1.0f, x0, w);
+          m = strip_bin_weights(geo.z, geo.w, pw, sampling_grid(g, geo.w), W, 1.0f, x0, w);
           float4* dst = reinterpret_cast<float4*>(s_xw + (c * PW + pw) * 8);
           dst[0] = make_float4(w[0], w[1], w[2], w[3]);
           dst[1] = make_float4(w[4], w[5], w[6], w[7]);
@@ -463,8 +465,7 @@ struct StripPlan {
 
 static int strip_plan(const LevelsParam& lv, const RoiArgs& a, const int64_t* gs, size_t esz, StripPlan* pl) {
   StripLevels& t = pl->sl;
-  if (a.sampling_ratio <= 0) return RAF_ERR_UNSUPPORTED;
-  if (a.PH > 32 || a.PW > 32) return RAF_ERR_UNSUPPORTED;
+  if (a.sampling_ratio < 0 || a.PH > 32 || a.PW > 32) return RAF_ERR_UNSUPPORTED;
   memset(&t, 0, sizeof(t));
   t.L = lv.L; t.N = lv.n; t.C = lv.c;
   t.chunks = (lv.c + 255) / 256;

@@ -52,6 +52,14 @@ __device__ __forceinline__ int batch_index_of(float f, int N) {
   return ((float)i == f) ? i : -1;
 }
 
+// Samples per bin along one axis: the fixed grid, or (reading S7, sampling_ratio == 0) ceil(bin size),
+// 0 for a non-positive / NaN bin size, capped at kMaxAdaptiveGrid.
+__device__ __forceinline__ int sampling_grid(int sampling_ratio, float bin) {
+  if (sampling_ratio > 0) return sampling_ratio;
+  const float c = ceilf(bin);
+  return (c >= (float)kMaxAdaptiveGrid) ? kMaxAdaptiveGrid : ((c >= 1.0f) ? (int)c : 0);
+}
+
 // C3, first block: geometry of one RoI on its level.
 struct RoiGeom {
   float sx, sy, bw, bh;
@@ -77,14 +85,8 @@ __device__ __forceinline__ RoiGeom roi_geom(float x1, float y1, float x2, float 
   g.sy = sy;
   g.bw = __fdiv_rn(rw, (float)PW);
   g.bh = __fdiv_rn(rh, (float)PH);
-  if (sampling_ratio > 0) {
-    g.gh = sampling_ratio;
-    g.gw = sampling_ratio;
-  } else {  // reading S7: adaptive grid
-    const float ch = ceilf(g.bh), cw = ceilf(g.bw);
-    g.gh = (ch >= (float)kMaxAdaptiveGrid) ? kMaxAdaptiveGrid : ((ch >= 1.0f) ? (int)ch : 0);
-    g.gw = (cw >= (float)kMaxAdaptiveGrid) ? kMaxAdaptiveGrid : ((cw >= 1.0f) ? (int)cw : 0);
-  }
+  g.gh = sampling_grid(sampling_ratio, g.bh);
+  g.gw = sampling_grid(sampling_ratio, g.bw);
   const int cnt = g.gh * g.gw;
   g.inv_count = 1.0f / (float)(cnt > 1 ? cnt : 1);
   return g;

@@ -31,6 +31,7 @@ struct FwdTap {
 #define RAF_FWD_MINB 3
 #endif
 constexpr int kFwdWarps = 8;   // max warps per CTA (one output bin row each, strided)
+constexpr int kFwdAdaptGrid = 8;   // adaptive sampling: grids up to 8 per axis are tabulated (16 tap slots per bin)
 
 // Merged taps of bin `bin` of one axis into tab[0..2g) (shared memory); returns the count.
 // Equal pixels are merged (weights summed in sample order); invalid samples (reading S6) give no tap.
@@ -96,8 +97,17 @@ __device__ __forceinline__ void fwd_accumulate(const T* rp0, const T* rp1, const
 #pragma unroll
     for (int b = 0; b < NX; ++b) {
       const float w = yw[a] * xw[b];
+#ifndef RAF_NO_FFMA2
+      const float2 ww = make_float2(w, w);   // packed fp32x2 FMAs (sm_100): one issue slot per two channels
+#pragma unroll
+      for (int j = 0; j < VN; j += 2) {
+        const float2 r = __ffma2_rn(ww, make_float2(v[a][b][j], v[a][b][j + 1]), make_float2(acc[j], acc[j + 1]));
+        acc[j] = r.x; acc[j + 1] = r.y;
+      }
+#else
 #pragma unroll
       for (int j = 0; j < VN; ++j) acc[j] = fmaf(w, v[a][b][j], acc[j]);
+#endif
     }
 }
 
@@ -110,6 +120,44 @@ __device__ __forceinline__ void fwd_dispatch_x(int nx, const T* rp0, const T* rp
     case 2: fwd_accumulate<T, NY, 2>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
     case 3: fwd_accumulate<T, NY, 3>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
     default: fwd_accumulate<T, NY, 4>(rp0, rp1, rp2, rp3, yw, xo, xw, acc); break;
+  }
+}
+
+// Adaptive grids beyond the tables: one warp per bin row, lanes = channel vectors, every sample evaluated as C3
+// writes it (rare: bins wider than kFwdAdaptGrid pixels).
+template <typename T>
+__device__ __noinline__ void fwd_direct_rows(const RoiGeom geo, const T* base, T* out_k, int b, int H, int W, int sh, int sw,
+                                             int PW, int ph0, int rend, int nwarps, int64_t os_h, int64_t os_w) {
+  using V = Vec16<T>;
+  constexpr int VN = V::N;
+  for (int ph = ph0; ph < rend; ph += nwarps) {
+    for (int pw = 0; pw < PW; ++pw) {
+      float acc[VN];
+#pragma unroll
+      for (int j = 0; j < VN; ++j) acc[j] = 0.0f;
+      if (b >= 0) {
+        for (int iy = 0; iy < geo.gh; ++iy) {
+          const AxisTap ty = axis_tap(sample_coord(geo.sy, geo.bh, ph, iy, geo.gh), H);
+          if (!ty.valid) continue;
+          for (int ix = 0; ix < geo.gw; ++ix) {
+            const AxisTap tx = axis_tap(sample_coord(geo.sx, geo.bw, pw, ix, geo.gw), W);
+            if (!tx.valid) continue;
+            const float w4[4] = {ty.wh * tx.wh, ty.wh * tx.wl, ty.wl * tx.wh, ty.wl * tx.wl};
+            const int o4[4] = {ty.lo * sh + tx.lo * sw, ty.lo * sh + tx.hi * sw, ty.hi * sh + tx.lo * sw, ty.hi * sh + tx.hi * sw};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              float v[VN];
+              V::load(base + o4[q], v);
+#pragma unroll
+              for (int j = 0; j < VN; ++j) acc[j] = fmaf(w4[q], v[j], acc[j]);
+            }
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < VN; ++j) acc[j] *= geo.inv_count;
+      }
+      V::store(out_k + ph * os_h + pw * os_w, acc);
+    }
   }
 }
 
@@ -127,7 +175,10 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   using V = Vec16<T>;
   constexpr int VN = V::N;
   extern __shared__ __align__(16) unsigned char fwd_smem[];
-  const int g = a.sampling_ratio, slots = 2 * g;
+  // sampling_ratio == 0 (adaptive grid, reading S7): the grid is per RoI, gh = ceil(bin height), gw likewise;
+  // the tables take grids up to kFwdAdaptGrid per axis, larger ones (bins wider than 8 pixels: boxes far
+  // beyond what the level map assigns) are sampled directly
+  const int g = a.sampling_ratio, slots = g > 0 ? 2 * g : 2 * kFwdAdaptGrid;
   const int PH = a.PH, PW = a.PW, nb = PH + PW;
   FwdTap* s_tab = reinterpret_cast<FwdTap*>(fwd_smem);          // [PH + PW][slots]; y bins first
   int* s_cnt = reinterpret_cast<int*>(s_tab + nb * slots);     // [PH + PW]
@@ -150,12 +201,15 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   const float r0 = __ldg(r), x1 = __ldg(r + 1), y1 = __ldg(r + 2), x2 = __ldg(r + 3), y2 = __ldg(r + 4);
   const int level = level_of(x1, y1, x2, y2, lv.L, a.finest_scale);
 
+  RoiGeom geo{};
+  if (g == 0 || (int)threadIdx.x < nb) geo = roi_geom(x1, y1, x2, y2, lv.scale[level], PH, PW, g, a.aligned);
+  const bool direct = g == 0 && (geo.gh > kFwdAdaptGrid || geo.gw > kFwdAdaptGrid);   // (uniform over the CTA)
   if ((int)threadIdx.x < nb) {
     const int t = threadIdx.x;
-    const RoiGeom geo = roi_geom(x1, y1, x2, y2, lv.scale[level], PH, PW, g, a.aligned);
     const bool isy = t < PH;
-    s_cnt[t] = isy ? fwd_bin_taps(geo.sy, geo.bh, t, g, lv.h[level], (int)lv.sh[level], geo.inv_count, s_tab + t * slots)
-                   : fwd_bin_taps(geo.sx, geo.bw, t - PH, g, lv.w[level], (int)lv.sw[level], 1.0f, s_tab + t * slots);
+    if (!direct)
+      s_cnt[t] = isy ? fwd_bin_taps(geo.sy, geo.bh, t, geo.gh, lv.h[level], (int)lv.sh[level], geo.inv_count, s_tab + t * slots)
+                     : fwd_bin_taps(geo.sx, geo.bw, t - PH, geo.gw, lv.w[level], (int)lv.sw[level], 1.0f, s_tab + t * slots);
     if (t == 0) s_b = batch_index_of(r0, lv.n);
   }
   __syncthreads();
@@ -165,6 +219,12 @@ fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_
   if (cv * VN >= lv.c) return;
   T* out_k = out + (int64_t)k * os_k + cv * VN;
   const T* base = reinterpret_cast<const T*>(lv.data[level]) + (int64_t)(b >= 0 ? b : 0) * lv.sn[level] + cv * VN;
+
+  if (direct) {   // rare: sample by sample (C3 as written); kept out of line so that it costs the hot path no registers
+    fwd_direct_rows<T>(geo, base, out_k, b, lv.h[level], lv.w[level], (int)lv.sh[level], (int)lv.sw[level], PW, rbeg + warp,
+                       rend, nwarps, os_h, os_w);
+    return;
+  }
 
   for (int ph = rbeg + warp; ph < rend; ph += nwarps) {
     const int ny = (b >= 0) ? s_cnt[ph] : 0;
@@ -265,10 +325,10 @@ static int forward_typed(const LevelsParam& lv, const RoiArgs& a, void* out, con
                          bool channels_last, const PullPrepOut* prep, cudaStream_t stream) {
   T* o = reinterpret_cast<T*>(out);
   const int g = a.sampling_ratio;
-  if (channels_last && g > 0) {
+  if (channels_last) {
     const int CV = lv.c / Vec16<T>::N;
     const int chunks = (CV + 31) / 32;
-    size_t smem = (size_t)(a.PH + a.PW) * (2 * g * sizeof(FwdTap) + sizeof(int));
+    size_t smem = (size_t)(a.PH + a.PW) * (2 * (g > 0 ? g : kFwdAdaptGrid) * sizeof(FwdTap) + sizeof(int));
     // one warp per bin row: outputs taller than 8 rows are split over several CTAs of equal height
     // (14 rows: 2 x 7 warps -- measured 33.7 us vs 43.4 us for one CTA of 8 warps on config 4; splitting
     // 7-row outputs into 4 + 3 rows is slower: 43.4 us vs 39.6 us on config 3)

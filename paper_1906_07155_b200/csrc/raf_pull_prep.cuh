@@ -29,6 +29,7 @@ struct PullPrepOut {
 };
 
 __host__ __device__ inline int pull_prep_blocks(const RoiArgs& a, int nthreads) {
+  if (a.sampling_ratio <= 0) return 1;   // adaptive grid: no tap tables (only the strip backward takes it), buckets only
   const int64_t items = (int64_t)a.K * (a.PH + a.PW);
   return 1 + (int)((items + nthreads - 1) / nthreads);
 }
@@ -117,10 +118,11 @@ __device__ __forceinline__ void pull_taps_item(const LevelsParam& lv, const RoiA
 // last sample (with slack for that rounding) bound all of them; a sample at v touches
 // floor(max(v,0)) and the next pixel (clamped to n-1); samples outside [-1, n] touch nothing.
 __device__ __forceinline__ void axis_window(float start, float bin, int P, int g, int n, int& lo, int& hi) {
+  lo = 0x7fffffff; hi = -1;
+  if (g <= 0) return;   // adaptive grid of a box with no extent: no samples
   const float va = sample_coord(start, bin, 0, 0, g), vb = sample_coord(start, bin, P - 1, g - 1, g);
   const float slack = 0.01f + 1e-6f * fmaxf(fabsf(va), fabsf(vb));
   const float vlo = fminf(va, vb) - slack, vhi = fmaxf(va, vb) + slack;
-  lo = 0x7fffffff; hi = -1;
   if (!(vlo <= vhi) || vhi < -1.0f || vlo > (float)n) return;   // NaN or entirely outside
   lo = (int)fminf(fmaxf(vlo, 0.0f), (float)(n - 1));
   hi = min(n - 1, (int)fminf(fmaxf(vhi, 0.0f), (float)(n - 1)) + 1);
@@ -134,7 +136,8 @@ __device__ __forceinline__ void pull_prep_block(const LevelsParam& lv, const Roi
   int32_t* __restrict__ bperm = o.bperm;
   int32_t* __restrict__ boff = o.boff;
   int4* __restrict__ bwin = o.bwin;
-  if (block > 0) {           // blocks 1.. : tap tables (independent of the bucketing)
+  if (block > 0) {           // blocks 1.. : tap tables (independent of the bucketing; fixed grids only)
+    if (a.sampling_ratio <= 0) return;
     const int64_t idx = (int64_t)(block - 1) * nthreads + threadIdx.x;
     if (idx < (int64_t)a.K * (a.PH + a.PW)) pull_taps_item(lv, a, idx, o.taps);
     return;
@@ -213,8 +216,8 @@ __device__ __forceinline__ void pull_prep_block(const LevelsParam& lv, const Roi
         const int level = key / N;
         const RoiGeom geo = roi_geom(r[1], r[2], r[3], r[4], lv.scale[level], a.PH, a.PW, a.sampling_ratio, a.aligned);
         int4 w;
-        axis_window(geo.sy, geo.bh, a.PH, a.sampling_ratio, lv.h[level], w.x, w.y);
-        axis_window(geo.sx, geo.bw, a.PW, a.sampling_ratio, lv.w[level], w.z, w.w);
+        axis_window(geo.sy, geo.bh, a.PH, geo.gh, lv.h[level], w.x, w.y);
+        axis_window(geo.sx, geo.bw, a.PW, geo.gw, lv.w[level], w.z, w.w);
         if (w.x > w.y || w.z > w.w) w = make_int4(0x7fffffff, -1, 0x7fffffff, -1);
         bwin[p] = w;
         if (o.bgeo) o.bgeo[p] = make_float4(geo.sy, geo.bh, geo.sx, geo.bw);

@@ -100,6 +100,31 @@ def test_forward_variants(P, g, aligned, layout):
     _fwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned)
 
 
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_adaptive_large_grids_forward_and_backward(dtype):
+    """sampling_ratio = 0 with bins of up to ~30 pixels (grids far beyond the 8 x 8 the forward tabulates: its
+    sample-by-sample path) next to small boxes (grid 1) and boxes with no extent (grid 0, reading S7), on one
+    60 x 70 map: forward, and the deterministic strip backward with its per-RoI grids."""
+    rng = np.random.default_rng(21)
+    K, C, H, W = 40, 24, 60, 70
+    side = np.exp(rng.uniform(np.log(0.5), np.log(220.0), (K, 2)))
+    cx, cy = rng.uniform(-5, W + 5, K), rng.uniform(-5, H + 5, K)
+    rois = np.stack([np.zeros(K), cx - side[:, 0] / 2, cy - side[:, 1] / 2, cx + side[:, 0] / 2,
+                     cy + side[:, 1] / 2], 1).astype(np.float32)
+    rois[3, 3] = rois[3, 1]            # zero width: gw = 0 -> no samples
+    rois[5, 2], rois[5, 4] = rois[5, 4], rois[5, 2]   # reversed rows
+    feats = [rng.standard_normal((1, C, H, W)).astype(np.float32)]
+    dev, exact = T.device_feats(feats, dtype, "cl")
+    got = T.gpu_forward(dev, [1.0], rois, (7, 7), 0, True, 56.0, "cl")
+    ref = R.forward(exact, [1.0], rois, (7, 7), 0, True, 56.0, coord_f32=True)
+    T.assert_forward_close(got, ref, dtype)
+    gout = rng.standard_normal((K, C, 7, 7)).astype(np.float32)
+    for flags in (0, B.RAF_DETERMINISTIC, B.RAF_ATOMIC):
+        gg, go_exact = T.gpu_backward([(1, C, H, W)], [1.0], gout, rois, 0, True, 56.0, "cl", dtype, flags)
+        gref, S = R.backward([(1, C, H, W)], [1.0], go_exact, rois, (7, 7), 0, True, 56.0)
+        T.assert_backward_close(gg, gref, S)
+
+
 def test_forward_degenerate_and_invalid_rois():
     wl = inputs.make_workload(2, n_img=2, per_img=8, channels=16)
     rois = np.array([[0, 100, 100, 100, 100], [1, 300, 200, 100, 50], [0, -500, -500, -400, -400],
@@ -191,17 +216,13 @@ def test_backward_reduced_configs(index, dtype, kw, layout, flags):
     _bwd_case(inputs.make_workload(index, **kw), dtype, layout, flags=flags)
 
 
-@pytest.mark.parametrize("layout,flags", [("cl", 0), ("cl", B.RAF_ATOMIC), ("cl", B.RAF_PULL_STRIP), ("nchw", 0)])
+@pytest.mark.parametrize("layout,flags", [("cl", 0), ("cl", B.RAF_ATOMIC), ("cl", B.RAF_PULL_STRIP),
+                                          ("cl", B.RAF_DETERMINISTIC), ("nchw", 0)])
 @pytest.mark.parametrize("P,g,aligned", [((7, 7), 1, True), ((7, 7), 0, True), ((7, 7), 2, False),
                                          ((5, 9), 3, True), ((14, 14), 2, True), ((7, 7), 0, False),
                                          ((32, 32), 2, True), ((1, 1), 4, True), ((3, 2), 16, False)])
 def test_backward_variants(P, g, aligned, layout, flags):
     wl = inputs.make_workload(5, n_img=2, per_img=24, channels=8)
-    if flags == B.RAF_PULL_STRIP and g == 0:   # the pull kernels need a fixed sampling grid: refused, not downgraded
-        with pytest.raises(B.RafError) as e:
-            _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned, flags=flags)
-        assert e.value.status == -5
-        return
     _bwd_case(wl, "f32", layout, P=P, g=g, aligned=aligned, flags=flags)
 
 

@@ -37,8 +37,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (1-based)")
     ap.add_argument("--layout", default="cl", choices=["cl", "nchw"])
-    ap.add_argument("--backward", default="auto", choices=["auto", "atomic", "deterministic"],
-                    help="auto: library's choice (pull when eligible); atomic: RAF_ATOMIC; deterministic: RAF_DETERMINISTIC")
+    ap.add_argument("--backward", default="auto", choices=["auto", "atomic", "deterministic", "strip", "tile"],
+                    help="auto: library's choice (a pull kernel when eligible); atomic: RAF_ATOMIC; deterministic: RAF_DETERMINISTIC; "
+                         "strip / tile: force one of the two pull kernels (RAF_PULL_STRIP / RAF_PULL_TILE)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--graph", action="store_true", help="replay each step from a CUDA graph")
@@ -277,8 +278,9 @@ def run_ours(args):
         g = args.sampling_ratio
     if args.aligned is not None:
         aligned = bool(args.aligned)
-    flags = {"auto": 0, "atomic": B.RAF_ATOMIC, "deterministic": B.RAF_DETERMINISTIC}[args.backward]
-    reuse = cfg.backward and not args.no_reuse_prep and args.backward != "atomic" and g > 0
+    flags = {"auto": 0, "atomic": B.RAF_ATOMIC, "deterministic": B.RAF_DETERMINISTIC, "strip": B.RAF_PULL_STRIP,
+             "tile": B.RAF_PULL_TILE}[args.backward]
+    reuse = cfg.backward and not args.no_reuse_prep and args.backward != "atomic"
     if reuse:
         flags |= B.RAF_REUSE_PREP   # a step runs the forward first, on the same RoIs and workspace: its launch
                                     # already wrote the backward's RoI buckets / tap tables (include/raf.h)

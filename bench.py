@@ -40,6 +40,8 @@ def parse_args():
     ap.add_argument("--backward", default="auto", choices=["auto", "atomic", "deterministic", "strip", "tile"],
                     help="auto: library's choice (a pull kernel when eligible); atomic: RAF_ATOMIC; deterministic: RAF_DETERMINISTIC; "
                          "strip / tile: force one of the two pull kernels (RAF_PULL_STRIP / RAF_PULL_TILE)")
+    ap.add_argument("--repack", action="store_true",
+                    help="with --layout nchw: RAF_REPACK (the library repacks to channels-last inside the workspace, counted in the time)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--graph", action="store_true", help="replay each step from a CUDA graph")
@@ -300,7 +302,13 @@ def run_ours(args):
     gouts = [lay(torch.from_numpy(wl.grad_out).to(tdt).cuda()) for _ in range(R)] if cfg.backward else None
     grads = [[lay(torch.empty(s, dtype=torch.float32, device="cuda")) for s in cfg.level_shapes]
              for _ in range(R)] if cfg.backward else None
-    ws = torch.empty(B.roi_align_fpn_workspace_bytes(K, L, PH, PW, g, flags), dtype=torch.uint8, device="cuda")
+    ws_bytes = B.roi_align_fpn_workspace_bytes(K, L, PH, PW, g, flags)
+    repack = bool(args.repack and args.layout == "nchw")
+    if repack:   # the library repacks NCHW <-> channels-last inside the (larger) workspace, inside every timed call
+        ws_bytes += B.roi_align_fpn_repack_bytes(feats[0], cfg.scales, tdt, K, PH, PW)
+        flags |= B.RAF_REPACK
+        fwd_flags |= B.RAF_REPACK
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
     fdesc = [B.make_levels(f, cfg.scales) for f in feats]
     gdesc = [B.make_levels(gr, cfg.scales) for gr in grads] if cfg.backward else None
     stream = torch.cuda.current_stream()
@@ -400,7 +408,7 @@ def run_ours(args):
         fp = {"level_hist": None}
         ab = {"fwd": pyr_bytes * esz + K * C * PH * PW * esz + 20 * K, "bwd": K * C * PH * PW * esz + pyr_bytes * 4}
     peak, peak_src = peaks()
-    variant = f"{args.layout}:{args.backward}:{'reuse' if reuse else 'noreuse'}"
+    variant = f"{args.layout}{'+repack' if repack else ''}:{args.backward}:{'reuse' if reuse else 'noreuse'}"
     traffic, traffic_stale = ncu_traffic(args.config, variant)
     legs = {"fwd": (ab["fwd"], loops["fwd"]["median_ms"])}
     if cfg.backward:
@@ -434,7 +442,7 @@ def run_ours(args):
                        "l2_protocol": (f"inputs rotate over {R} independent copies ({R * ws_set / 1e6:.0f} MB >> L2 {l2 / 1e6:.0f} MB)"
                                        if R * ws_set >= 2 * l2 else
                                        f"WARM: {R} buffer set(s), {R * ws_set / 1e6:.0f} MB vs L2 {l2 / 1e6:.0f} MB (not the headline)"),
-                       "backward": args.backward if cfg.backward else "none",
+                       "backward": args.backward if cfg.backward else "none", "repack": repack,
                        "reuse_prep": bool(reuse), "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
             "roofline": roof(dom),
             "roofline_all": {k: roof(k) for k in legs} | {"step": {

@@ -86,6 +86,17 @@ enum {
   RAF_NO_PREP = 16        /* forward only (inference): do not write the backward's prep tables; the
                              workspace is not touched and `ws` may be NULL                           */
 };
+/* Forward and backward flag: NCHW-contiguous operands (every level dense [N,C,H,W], out / grad_out dense
+ * [K,C,out_h,out_w]) are REPACKED to channels-last inside the workspace, the channels-last kernels run on the
+ * copies, and the result is repacked back -- all on `stream`, all inside the call ("any NCHW -> channel-last
+ * repack counted in the timing", north_star).  `ws` must then hold roi_align_fpn_workspace_bytes(...) +
+ * roi_align_fpn_repack_bytes(...) bytes (else RAF_ERR_WORKSPACE).  Ignored when the operands already are
+ * channels-last; RAF_ERR_STRIDE when they are neither.  Without the flag NCHW runs on the strided
+ * thread-per-element kernels (no extra memory, about 2.5x slower). */
+enum { RAF_REPACK = 128 };
+/* Bytes of channels-last scratch RAF_REPACK needs for these levels and this RoI tensor (the larger of the
+ * forward's and the backward's need; 256-aligned).  `levels`: HOST array, only the shapes are read. */
+size_t roi_align_fpn_repack_bytes(const raf_level* levels, int L, raf_dtype dtype, int K, int out_h, int out_w);
 /* With neither RAF_DETERMINISTIC nor RAF_ATOMIC the library picks the pull variant when eligible
  * and the atomic variant otherwise. */
 
@@ -128,7 +139,7 @@ int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, con
  *                shapes as the features.  Overwritten (every element written: zero or sum) unless
  *                RAF_ACCUMULATE.
  *   grad_out     DEVICE, dtype = gout_dtype, logical [K,C,out_h,out_w] through gout_strides (HOST)
- *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE */
+ *   flags        RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE | RAF_REPACK */
 int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
                            const void* grad_out, const int64_t* gout_strides, const float* rois,
                            int K, int out_h, int out_w, int sampling_ratio, int aligned,

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "libraf.so")
 
 RAF_F32, RAF_F16, RAF_BF16 = 0, 1, 2
 RAF_ACCUMULATE, RAF_DETERMINISTIC, RAF_ATOMIC, RAF_REUSE_PREP, RAF_NO_PREP = 1, 2, 4, 8, 16
-RAF_PULL_STRIP, RAF_PULL_TILE = 32, 64
+RAF_PULL_STRIP, RAF_PULL_TILE, RAF_REPACK = 32, 64, 128
 RAF_SOFT_LINEAR, RAF_SOFT_GAUSSIAN = 1, 2
 _DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_BF16}
 
@@ -25,6 +25,7 @@ EXPORTS = [
     "roi_align_fpn_forward_ex", "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
     "roi_pool_fpn_forward", "roi_pool_fpn_backward", "roi_nms_workspace_bytes", "roi_nms", "roi_soft_nms",
+    "roi_align_fpn_repack_bytes",
 ]
 
 
@@ -54,6 +55,8 @@ def lib() -> ctypes.CDLL:
         L = ctypes.CDLL(LIB_PATH)
         L.roi_align_fpn_workspace_bytes.restype = ctypes.c_size_t
         L.roi_align_fpn_workspace_bytes.argtypes = [ctypes.c_int] * 6
+        L.roi_align_fpn_repack_bytes.restype = ctypes.c_size_t
+        L.roi_align_fpn_repack_bytes.argtypes = [ctypes.c_void_p] + [ctypes.c_int] * 5
         L.roi_align_fpn_host_arena_bytes.restype = ctypes.c_size_t
         L.roi_align_fpn_host_arena_bytes.argtypes = [ctypes.c_void_p] + [ctypes.c_int] * 7
         L.roi_fpn_assign_levels.restype = ctypes.c_int
@@ -128,6 +131,13 @@ def _strides4(t: torch.Tensor):
 def roi_align_fpn_workspace_bytes(K: int, L: int, out_h: int, out_w: int, sampling_ratio: int,
                                   flags: int = 0) -> int:
     return int(lib().roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
+
+
+def roi_align_fpn_repack_bytes(levels: Sequence[torch.Tensor], scales: Sequence[float], dtype, K: int, out_h: int,
+                               out_w: int) -> int:
+    """Extra workspace bytes RAF_REPACK needs (append them to roi_align_fpn_workspace_bytes)."""
+    desc = make_levels(levels, scales)
+    return int(lib().roi_align_fpn_repack_bytes(desc, len(levels), _DTYPES[dtype], K, out_h, out_w))
 
 
 def roi_fpn_assign_levels(rois: torch.Tensor, L: int, finest_scale: float,

@@ -84,6 +84,16 @@ static bool level_dense(const raf_level& v) {
   return true;
 }
 
+// Dense NCHW (strides of extent-1 dimensions are not looked at).
+static bool level_nchw(const raf_level& v) {
+  return (v.w <= 1 || v.sw == 1) && (v.h <= 1 || v.sh == v.w) && (v.c <= 1 || v.sc == (int64_t)v.h * v.w) &&
+         (v.n <= 1 || v.sn == (int64_t)v.c * v.h * v.w);
+}
+static bool tensor_nchw(int K, int C, int PH, int PW, const int64_t* s) {
+  return (PW <= 1 || s[3] == 1) && (PH <= 1 || s[2] == PW) && (C <= 1 || s[1] == (int64_t)PH * PW) &&
+         (K <= 1 || s[0] == (int64_t)C * PH * PW);
+}
+
 }  // namespace raf
 
 using namespace raf;
@@ -177,6 +187,29 @@ int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, i
   return launch_assign_levels(rois, K, L, finest_scale, levels, counts, perm, (cudaStream_t)stream);
 }
 
+size_t roi_align_fpn_repack_bytes(const raf_level* levels, int L, raf_dtype dtype, int K, int out_h, int out_w) {
+  (void)dtype;   // sized for fp32 copies: the backward's gradient pyramid is fp32 whatever the feature dtype
+  if (!levels || L < 1 || L > kMaxLevels || K < 0 || out_h < 1 || out_w < 1) return 0;
+  size_t total = 256;
+  for (int l = 0; l < L; ++l) total += align256((size_t)levels[l].n * levels[l].c * levels[l].h * levels[l].w * 4);
+  total += align256((size_t)K * levels[0].c * out_h * out_w * 4);
+  return total;
+}
+
+// RAF_REPACK: channels-last descriptors of the scratch copies of dense NCHW levels, carved from `scratch`.
+static char* repack_levels(const raf_level* src, int L, size_t esz, char* scratch, raf_level* dst) {
+  for (int l = 0; l < L; ++l) {
+    dst[l] = src[l];
+    dst[l].data = scratch;
+    dst[l].sc = 1;
+    dst[l].sw = src[l].c;
+    dst[l].sh = (int64_t)src[l].w * src[l].c;
+    dst[l].sn = (int64_t)src[l].h * src[l].w * src[l].c;
+    scratch += align256((size_t)src[l].n * src[l].c * src[l].h * src[l].w * esz);
+  }
+  return scratch;
+}
+
 int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
                           int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
                           void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,
@@ -199,7 +232,34 @@ int roi_align_fpn_forward_ex(const raf_level* feats, int L, raf_dtype dtype, con
   if (K == 0) return RAF_OK;  // nothing to do; strides of an empty tensor are not meaningful
   for (int i = 0; i < 4; ++i) if (out_strides[i] <= 0) return RAF_ERR_STRIDE;
   if (!out) return RAF_ERR_NULL;
-  if (flags & ~RAF_NO_PREP) return RAF_ERR_UNSUPPORTED;
+  if (flags & ~(RAF_NO_PREP | RAF_REPACK)) return RAF_ERR_UNSUPPORTED;
+  if (flags & RAF_REPACK) {
+    const int vec0 = (int)(16 / esize(dtype));
+    const bool cl0 = levels_vectorizable(feats, L, vec0, esize(dtype)) &&
+                     tensor_vectorizable(out, out_strides, vec0, esize(dtype), K, out_h, out_w);
+    if (!cl0) {   // repack NCHW -> channels-last inside the workspace, run the fast path, repack the result back
+      for (int l = 0; l < L; ++l) if (!level_nchw(feats[l])) return RAF_ERR_STRIDE;
+      if (!tensor_nchw(K, feats[0].c, out_h, out_w, out_strides) || feats[0].c % vec0) return RAF_ERR_STRIDE;
+      const size_t base = roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, 0);
+      if (!ws) return RAF_ERR_NULL;
+      if ((uintptr_t)ws % 256) return RAF_ERR_WORKSPACE;
+      if (ws_bytes < base + roi_align_fpn_repack_bytes(feats, L, dtype, K, out_h, out_w)) return RAF_ERR_WORKSPACE;
+      cudaStream_t st = (cudaStream_t)stream;
+      raf_level cl_lv[kMaxLevels];
+      char* cur = repack_levels(feats, L, esize(dtype), (char*)ws + base, cl_lv);
+      void* cl_out = cur;
+      for (int l = 0; l < L; ++l) {
+        rc = launch_transpose(feats[l].data, cl_lv[l].data, feats[l].n, feats[l].c, feats[l].h * feats[l].w, esize(dtype), st);
+        if (rc) return rc;
+      }
+      const int C = feats[0].c;
+      const int64_t cl_strides[4] = {(int64_t)out_h * out_w * C, 1, (int64_t)out_w * C, C};
+      rc = roi_align_fpn_forward_ex(cl_lv, L, dtype, rois, K, out_h, out_w, sampling_ratio, aligned, finest_scale, cl_out,
+                                    cl_strides, flags & ~RAF_REPACK, ws, base, stream);
+      if (rc) return rc;
+      return launch_transpose(cl_out, out, K, out_h * out_w, C, esize(dtype), st);
+    }
+  }
   const bool want_prep = !(flags & RAF_NO_PREP);
   if (want_prep) {
     if (!ws) return RAF_ERR_NULL;
@@ -231,7 +291,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (rc) return rc;
   if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
-  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE)) return RAF_ERR_UNSUPPORTED;
+  if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE | RAF_REPACK)) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_PULL_STRIP) && (flags & (RAF_PULL_TILE | RAF_ATOMIC))) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_PULL_TILE) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
@@ -243,6 +303,36 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   if (ws_bytes < roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags))
     return RAF_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
+  if ((flags & RAF_REPACK) && K > 0) {
+    const bool cl0 = levels_vectorizable(grad_feats, L, 4, 4) &&
+                     tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype), K, out_h, out_w);
+    if (!cl0) {   // grad_out -> channels-last copy, fast backward into a channels-last gradient copy, repack back
+      for (int l = 0; l < L; ++l) if (!level_nchw(grad_feats[l])) return RAF_ERR_STRIDE;
+      const int C = grad_feats[0].c;
+      if (!tensor_nchw(K, C, out_h, out_w, gout_strides) || C % 4 || (esize(gout_dtype) == 2 && C % 8)) return RAF_ERR_STRIDE;
+      const size_t base = roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags);
+      if (ws_bytes < base + roi_align_fpn_repack_bytes(grad_feats, L, gout_dtype, K, out_h, out_w)) return RAF_ERR_WORKSPACE;
+      raf_level cl_lv[kMaxLevels];
+      char* cur = repack_levels(grad_feats, L, 4, (char*)ws + base, cl_lv);
+      void* cl_gout = cur;
+      rc = launch_transpose(grad_out, cl_gout, K, C, out_h * out_w, esize(gout_dtype), st);
+      if (rc) return rc;
+      if (flags & RAF_ACCUMULATE)
+        for (int l = 0; l < L; ++l) {
+          rc = launch_transpose(grad_feats[l].data, cl_lv[l].data, grad_feats[l].n, C, grad_feats[l].h * grad_feats[l].w, 4, st);
+          if (rc) return rc;
+        }
+      const int64_t cl_strides[4] = {(int64_t)out_h * out_w * C, 1, (int64_t)out_w * C, C};
+      rc = roi_align_fpn_backward(cl_lv, L, gout_dtype, cl_gout, cl_strides, rois, K, out_h, out_w, sampling_ratio, aligned,
+                                  finest_scale, flags & ~RAF_REPACK, ws, base, stream);
+      if (rc) return rc;
+      for (int l = 0; l < L; ++l) {
+        rc = launch_transpose(cl_lv[l].data, grad_feats[l].data, grad_feats[l].n, grad_feats[l].h * grad_feats[l].w, C, 4, st);
+        if (rc) return rc;
+      }
+      return RAF_OK;
+    }
+  }
   LevelsParam p;
   fill_param(grad_feats, L, &p);
   const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};

@@ -80,6 +80,9 @@ int launch_nms(const float* boxes, const float* scores, int n, float iou_thresho
 int launch_soft_nms(const float* boxes, const float* scores, int n, float iou_threshold, float sigma, float min_score,
                     int method, int32_t* keep, float* new_scores, int32_t* num_keep, void* ws, cudaStream_t stream);
 
+// Batched transpose src[batch][R][S] -> dst[batch][S][R] (raf_repack.cu): the NCHW <-> channels-last repack.
+int launch_transpose(const void* src, void* dst, int64_t batch, int R, int S, size_t esz, cudaStream_t stream);
+
 // Zero-fill of one strided level (used when the level is not one dense block).
 int launch_zero_level(float* data, int n, int c, int h, int w, int64_t sn, int64_t sc, int64_t sh,
                       int64_t sw, cudaStream_t stream);

@@ -602,3 +602,60 @@ def test_no_out_of_bounds_writes(index, dtype, kw, P, flags):
     for gb, nb in gbufs:
         assert _margins_intact(gb, nb), "backward wrote outside the gradient pyramid"
     assert all(torch.isfinite(g).all() for g in grads) and torch.isfinite(out.float()).all()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+def test_repack_nchw_forward_and_backward(dtype):
+    """RAF_REPACK: dense NCHW operands are repacked to channels-last inside the workspace,
+    the channels-last kernels run, the result is repacked back.  Must equal the channels-last call bit for bit
+    (same kernels on the same values) and the oracle within tolerance; NaN-filled destinations and a
+    garbage-filled workspace; accumulate mode repacks the existing gradients in first."""
+    wl = inputs.make_workload(5, n_img=2, per_img=40, channels=32)
+    cfg = wl.cfg
+    tdt = T.TORCH_DTYPE[dtype]
+    PH, PW = cfg.out_size
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    rois = torch.from_numpy(wl.rois).cuda()
+    f_nchw, exact = T.device_feats(wl.feats, dtype, "nchw")
+    f_cl, _ = T.device_feats(wl.feats, dtype, "cl")
+    base = B.roi_align_fpn_workspace_bytes(K, L, PH, PW, 2, 0)
+    extra = B.roi_align_fpn_repack_bytes(f_nchw, cfg.scales, tdt, K, PH, PW)
+    ws = torch.full((base + extra,), 0x7B, dtype=torch.uint8, device="cuda")
+    o_nchw = torch.full((K, C, PH, PW), float("nan"), dtype=tdt, device="cuda")
+    o_cl = T.empty_layout((K, C, PH, PW), tdt, "cl", fill=float("nan"))
+    B.roi_align_fpn_forward_ex(f_nchw, cfg.scales, rois, o_nchw, 2, True, cfg.finest_scale, B.RAF_REPACK, ws)
+    B.roi_align_fpn_forward(f_cl, cfg.scales, rois, o_cl, 2, True, cfg.finest_scale, T.workspace(K, L, PH, PW, 2))
+    torch.cuda.synchronize()
+    assert o_nchw.is_contiguous() and torch.equal(o_nchw, o_cl)
+    ref = R.forward(exact, cfg.scales, wl.rois, (PH, PW), 2, True, cfg.finest_scale, coord_f32=True)
+    T.assert_forward_close(o_nchw.to(torch.float64).cpu().numpy(), ref, dtype)
+    # a workspace without room for the copies is refused; so are operands that are neither layout
+    with pytest.raises(B.RafError) as e:
+        B.roi_align_fpn_forward_ex(f_nchw, cfg.scales, rois, o_nchw, 2, True, cfg.finest_scale, B.RAF_REPACK, ws[:base])
+    assert e.value.status == -6
+    with pytest.raises(B.RafError) as e:
+        B.roi_align_fpn_forward_ex([f[:, ::2] for f in f_nchw], cfg.scales, rois, o_nchw[:, ::2], 2, True,
+                                   cfg.finest_scale, B.RAF_REPACK, ws)
+    assert e.value.status == -4
+    # backward: overwrite, then accumulate on top of random gradients; RAF_REUSE_PREP works through the repack
+    go_t = torch.from_numpy(wl.grad_out).to(tdt)
+    go_nchw = go_t.cuda().contiguous()
+    go_cl = T.to_layout(go_t.cuda(), "cl")
+    rng = np.random.default_rng(5)
+    init = [rng.standard_normal(s).astype(np.float32) for s in cfg.level_shapes]
+    for flags, start in ((0, None), (B.RAF_ACCUMULATE, init), (B.RAF_REUSE_PREP, None)):
+        if start is None:
+            g_nchw = [torch.full(s, float("nan"), dtype=torch.float32, device="cuda") for s in cfg.level_shapes]
+            g_cl = [T.empty_layout(s, torch.float32, "cl", fill=float("nan")) for s in cfg.level_shapes]
+        else:
+            g_nchw = [torch.from_numpy(x).cuda().contiguous() for x in start]
+            g_cl = [T.to_layout(torch.from_numpy(x).cuda(), "cl") for x in start]
+        B.roi_align_fpn_backward(g_nchw, cfg.scales, go_nchw, rois, 2, True, cfg.finest_scale, flags | B.RAF_REPACK, ws)
+        B.roi_align_fpn_backward(g_cl, cfg.scales, go_cl, rois, 2, True, cfg.finest_scale, flags & ~B.RAF_REUSE_PREP,
+                                 T.workspace(K, L, PH, PW, 2))
+        torch.cuda.synchronize()
+        for a_, b_ in zip(g_nchw, g_cl):
+            assert a_.is_contiguous() and torch.equal(a_, b_)
+    gref, S = R.backward(cfg.level_shapes, cfg.scales, go_t.to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
+                         cfg.finest_scale)
+    T.assert_backward_close([t.to(torch.float64).cpu().numpy() for t in g_nchw], gref, S)

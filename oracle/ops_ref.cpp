@@ -2,7 +2,9 @@
 //   * multi-level (FPN) RoIPool-max forward / backward  ("RoIPooling-like operators", section
 //     3.1 RoIExtractor; the max variant is the RoI pooling layer of Fast R-CNN);
 //   * greedy NMS and Soft-NMS on boxes ("Soft NMS [1]: an alternative to NMS"; "All basic
-//     bbox and mask operations run on GPUs").
+//     bbox and mask operations run on GPUs");
+//   * deformable RoI pooling forward / backward ("DCN [8]: deformable convolution and deformable RoI pooling",
+//     PAPER.md:57-58): RoIAlign whose bins are shifted by per-bin offsets (readings D1-D5).
 //
 // THIS IS TEST INFRASTRUCTURE, NOT PRODUCT CODE.  Only tests/, __graft_entry__.smoke() and bench.py's
 // cpu_baseline / --impl reference legs may load it.  It shares no code, header, table or helper with the
@@ -20,7 +22,11 @@
 // recorded argmax (mass conservation, brute force).  NMS -- hand-worked 5-box example, threshold edge,
 // permutation invariance, brute-force O(n^2) restatement on tiny inputs via the library routine
 // torchvision.ops.nms, idempotence.  Soft-NMS -- hand-worked 3-box example (linear and Gaussian), reduction
-// to a score sort when no boxes overlap.  Nothing here is "parity unpinned".
+// to a score sort when no boxes overlap.  Deformable RoI pooling -- zero offsets == the RoIAlign oracle
+// (oracle/raf_ref.cpp, itself pinned) bit for bit; a uniform offset == RoIAlign of the translated box (f64
+// mode, 1e-12); an offset on one bin changes that bin only; adjoint identity for the feature gradient;
+// central finite differences of the f64 forward for the offset gradient; constant map -> zero offset
+// gradient.  Nothing here is "parity unpinned".
 #include <cfloat>
 #include <cmath>
 #include <cstdint>
@@ -214,6 +220,180 @@ int soft_nms_ref(const float* boxes, const float* scores, int n, float iou_thres
   delete[] s;
   delete[] gone;
   return nk;
+}
+
+
+}  // extern "C" (the templates below have C++ linkage; the two entry points re-open it)
+
+// ---- Deformable RoI pooling (D1-D5) --------------------------------------------------
+// D1: the RoI on its level as in C3 with the half-pixel shift and no minimum size ("aligned"):
+//       sx = x1*scale - 0.5, ex = x2*scale - 0.5, rw = ex - sx, bw = rw / PW   (rows likewise); level by C1.
+// D2: grid per axis g = sampling_ratio, or (sampling_ratio == 0) ceil(bin size), 0 for a non-positive size;
+//       count = max(gh*gw, 1).
+// D3: bin (ph, pw) of RoI k is shifted by  ox = (gamma*rw) * offset[k,0,ph,pw],  oy = (gamma*rh) * offset[k,1,ph,pw]
+//       (feature pixels; plane 0 = x, plane 1 = y; a NULL offset tensor = zeros); sample (iy, ix) sits at
+//       x = [(sx + pw*bw) + ((ix + 0.5)*bw)/gw] + ox,  y likewise  -- the C3 coordinate, then ONE more addition.
+//       Spec mode: all of this in fp32, each operation rounded, in this order; f64 mode: in double.
+// D4: every sample is a C3 bilinear sample (outside [-1,H] x [-1,W] -> contributes 0, count unchanged; clamped
+//       at 0 and at the last pixel); out = sum / count.
+// D5: backward.  Features: the exact transpose.  Offsets: the derivative of D3-D4 where it exists,
+//       d out / d offset_x = (gamma*rw) / count * sum_samples d val / d x,   d val / d x = (hy*(F[yl,xh]-F[yl,xl]) +
+//       ly*(F[yh,xh]-F[yh,xl])) for a valid sample whose x is not clamped (0 < x < W-1), 0 otherwise (the forward is
+//       constant in x there); y likewise.
+template <typename R>
+struct DeformTap {   // one axis of one sample
+  int lo, hi;
+  R wl, wh;      // weight of hi (fraction l) and of lo (1 - l)
+  bool valid;    // inside [-1, n]
+  bool inner;    // 0 < v < n-1 and lo < hi: the forward depends on v here
+};
+
+template <typename R>
+static DeformTap<R> deform_axis(R v, int n) {
+  DeformTap<R> t;
+  t.valid = (v >= (R)-1) && (v <= (R)n);
+  t.inner = t.valid && (v > (R)0);
+  if (!(v > (R)0)) v = (R)0;
+  int lo = t.valid ? (int)v : 0;
+  int hi;
+  if (lo >= n - 1) { lo = hi = n - 1; v = (R)lo; t.inner = false; }
+  else hi = lo + 1;
+  t.lo = lo; t.hi = hi;
+  t.wl = v - (R)lo;
+  t.wh = (R)1 - t.wl;
+  return t;
+}
+
+template <typename R>
+struct DeformGeom { R sx, sy, rw, rh, bw, bh; int gh, gw; int count; };
+
+template <typename R>
+static DeformGeom<R> deform_geom(const float* roi, float scale, int PH, int PW, int sampling_ratio) {
+  DeformGeom<R> g;
+  const R sc = (R)scale, half = (R)0.5;
+  g.sx = (R)roi[1] * sc - half; g.sy = (R)roi[2] * sc - half;
+  const R ex = (R)roi[3] * sc - half, ey = (R)roi[4] * sc - half;
+  g.rw = ex - g.sx; g.rh = ey - g.sy;
+  g.bw = g.rw / (R)PW; g.bh = g.rh / (R)PH;
+  auto grid = [&](R b) -> int {
+    if (sampling_ratio > 0) return sampling_ratio;
+    const R c = std::ceil(b);
+    return (c >= (R)1) ? (int)c : 0;
+  };
+  g.gh = grid(g.bh); g.gw = grid(g.bw);
+  const int cnt = g.gh * g.gw;
+  g.count = cnt > 1 ? cnt : 1;
+  return g;
+}
+
+template <typename R>
+static R deform_coord(R start, R bin, int p, int i, int grid, R shift) {
+  const R a = start + (R)p * bin;
+  const R d = (((R)i + (R)0.5) * bin) / (R)grid;
+  return (a + d) + shift;
+}
+
+template <typename R>
+static int deform_forward(const ops_ref_level* feats, int L, const float* rois, int K, const float* offset, float gamma,
+                          int PH, int PW, int sampling_ratio, float finest_scale, double* out) {
+  const int C = feats[0].c;
+  for (int k = 0; k < K; ++k) {
+    const float* roi = rois + 5 * (int64_t)k;
+    const int l = level_of(roi, L, finest_scale);
+    const ops_ref_level& lv = feats[l];
+    const int b = batch_index_of(roi[0], lv.n);
+    const DeformGeom<R> g = deform_geom<R>(roi, lv.spatial_scale, PH, PW, sampling_ratio);
+    for (int c = 0; c < C; ++c)
+      for (int ph = 0; ph < PH; ++ph)
+        for (int pw = 0; pw < PW; ++pw) {
+          double acc = 0.0;
+          if (b >= 0) {
+            const R dx = offset ? (R)offset[(((int64_t)k * 2 + 0) * PH + ph) * PW + pw] : (R)0;
+            const R dy = offset ? (R)offset[(((int64_t)k * 2 + 1) * PH + ph) * PW + pw] : (R)0;
+            const R ox = ((R)gamma * g.rw) * dx, oy = ((R)gamma * g.rh) * dy;
+            const double* F = lv.data + ((int64_t)b * C + c) * lv.h * lv.w;
+            for (int iy = 0; iy < g.gh; ++iy) {
+              const DeformTap<R> ty = deform_axis<R>(deform_coord<R>(g.sy, g.bh, ph, iy, g.gh, oy), lv.h);
+              if (!ty.valid) continue;
+              for (int ix = 0; ix < g.gw; ++ix) {
+                const DeformTap<R> tx = deform_axis<R>(deform_coord<R>(g.sx, g.bw, pw, ix, g.gw, ox), lv.w);
+                if (!tx.valid) continue;
+                const R w1 = ty.wh * tx.wh, w2 = ty.wh * tx.wl, w3 = ty.wl * tx.wh, w4 = ty.wl * tx.wl;
+                acc += (double)w1 * F[(int64_t)ty.lo * lv.w + tx.lo] + (double)w2 * F[(int64_t)ty.lo * lv.w + tx.hi] +
+                       (double)w3 * F[(int64_t)ty.hi * lv.w + tx.lo] + (double)w4 * F[(int64_t)ty.hi * lv.w + tx.hi];
+              }
+            }
+          }
+          out[(((int64_t)k * C + c) * PH + ph) * PW + pw] = acc / (double)g.count;
+        }
+  }
+  return 0;
+}
+
+extern "C" int deform_roi_pool_fpn_forward_ref(const ops_ref_level* feats, int L, const float* rois, int K, const float* offset,
+                                    float gamma, int PH, int PW, int sampling_ratio, float finest_scale, int f64_mode,
+                                    double* out) {
+  return f64_mode ? deform_forward<double>(feats, L, rois, K, offset, gamma, PH, PW, sampling_ratio, finest_scale, out)
+                  : deform_forward<float>(feats, L, rois, K, offset, gamma, PH, PW, sampling_ratio, finest_scale, out);
+}
+
+template <typename R>
+static int deform_backward(const ops_ref_level* feats, const ops_ref_level* grads, int L, const double* grad_out,
+                           const float* rois, int K, const float* offset, float gamma, int PH, int PW, int sampling_ratio,
+                           float finest_scale, double* grad_offset) {
+  const int C = feats[0].c;
+  if (grad_offset) memset(grad_offset, 0, sizeof(double) * (size_t)K * 2 * PH * PW);
+  for (int k = 0; k < K; ++k) {
+    const float* roi = rois + 5 * (int64_t)k;
+    const int l = level_of(roi, L, finest_scale);
+    const ops_ref_level& lv = feats[l];
+    const int b = batch_index_of(roi[0], lv.n);
+    if (b < 0) continue;
+    const DeformGeom<R> g = deform_geom<R>(roi, lv.spatial_scale, PH, PW, sampling_ratio);
+    for (int c = 0; c < C; ++c)
+      for (int ph = 0; ph < PH; ++ph)
+        for (int pw = 0; pw < PW; ++pw) {
+          const double go = grad_out[(((int64_t)k * C + c) * PH + ph) * PW + pw] / (double)g.count;
+          const R dx = offset ? (R)offset[(((int64_t)k * 2 + 0) * PH + ph) * PW + pw] : (R)0;
+          const R dy = offset ? (R)offset[(((int64_t)k * 2 + 1) * PH + ph) * PW + pw] : (R)0;
+          const R ox = ((R)gamma * g.rw) * dx, oy = ((R)gamma * g.rh) * dy;
+          const double* F = lv.data + ((int64_t)b * C + c) * lv.h * lv.w;
+          double* G = grads ? grads[l].data + ((int64_t)b * C + c) * lv.h * lv.w : nullptr;
+          double gx = 0.0, gy = 0.0;
+          for (int iy = 0; iy < g.gh; ++iy) {
+            const DeformTap<R> ty = deform_axis<R>(deform_coord<R>(g.sy, g.bh, ph, iy, g.gh, oy), lv.h);
+            if (!ty.valid) continue;
+            for (int ix = 0; ix < g.gw; ++ix) {
+              const DeformTap<R> tx = deform_axis<R>(deform_coord<R>(g.sx, g.bw, pw, ix, g.gw, ox), lv.w);
+              if (!tx.valid) continue;
+              const int64_t i1 = (int64_t)ty.lo * lv.w + tx.lo, i2 = (int64_t)ty.lo * lv.w + tx.hi;
+              const int64_t i3 = (int64_t)ty.hi * lv.w + tx.lo, i4 = (int64_t)ty.hi * lv.w + tx.hi;
+              if (G) {
+                G[i1] += (double)(ty.wh * tx.wh) * go; G[i2] += (double)(ty.wh * tx.wl) * go;
+                G[i3] += (double)(ty.wl * tx.wh) * go; G[i4] += (double)(ty.wl * tx.wl) * go;
+              }
+              if (tx.inner) gx += (double)ty.wh * (F[i2] - F[i1]) + (double)ty.wl * (F[i4] - F[i3]);
+              if (ty.inner) gy += (double)tx.wh * (F[i3] - F[i1]) + (double)tx.wl * (F[i4] - F[i2]);
+            }
+          }
+          if (grad_offset) {
+            grad_offset[(((int64_t)k * 2 + 0) * PH + ph) * PW + pw] += go * gx * (double)((R)gamma * g.rw);
+            grad_offset[(((int64_t)k * 2 + 1) * PH + ph) * PW + pw] += go * gy * (double)((R)gamma * g.rh);
+          }
+        }
+  }
+  return 0;
+}
+
+extern "C" {
+// grads (may be NULL: offsets only) must hold their starting values; grad_offset [K,2,PH,PW] (may be NULL) is overwritten.
+int deform_roi_pool_fpn_backward_ref(const ops_ref_level* feats, const ops_ref_level* grads, int L, const double* grad_out,
+                                     const float* rois, int K, const float* offset, float gamma, int PH, int PW,
+                                     int sampling_ratio, float finest_scale, int f64_mode, double* grad_offset) {
+  return f64_mode ? deform_backward<double>(feats, grads, L, grad_out, rois, K, offset, gamma, PH, PW, sampling_ratio,
+                                            finest_scale, grad_offset)
+                  : deform_backward<float>(feats, grads, L, grad_out, rois, K, offset, gamma, PH, PW, sampling_ratio,
+                                           finest_scale, grad_offset);
 }
 
 }  // extern "C"

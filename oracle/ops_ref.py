@@ -1,4 +1,4 @@
-"""ctypes front end of the CPU oracle for RoIPool-max, NMS and Soft-NMS (oracle/ops_ref.cpp).
+"""ctypes front end of the CPU oracle for RoIPool-max, NMS, Soft-NMS and deformable RoI pooling (oracle/ops_ref.cpp).
 
 TEST INFRASTRUCTURE, NOT PRODUCT CODE: only tests/, __graft_entry__.smoke() and bench.py's
 cpu_baseline / --impl reference legs may import this module.  It imports nothing from the product
@@ -97,3 +97,35 @@ def soft_nms(boxes, scores, iou_threshold, sigma, min_score, method):
     nk = lib().soft_nms_ref(_p(boxes), _p(scores), n, ctypes.c_float(iou_threshold), ctypes.c_float(sigma),
                             ctypes.c_float(min_score), {"linear": 1, "gaussian": 2}[method], _p(keep), _p(ns))
     return keep[:nk].copy(), ns[:nk].copy()
+
+
+def deform_roi_pool_forward(feats, scales, rois, offset, gamma, out_size, sampling_ratio=2, finest_scale=56.0, f64=False):
+    """D1-D4.  offset: float32 [K,2,PH,PW] (plane 0 = x, 1 = y) or None.  Returns float64 [K,C,PH,PW]."""
+    feats64 = [np.ascontiguousarray(f, dtype=np.float64) for f in feats]
+    rois = np.ascontiguousarray(rois, dtype=np.float32)
+    PH, PW = out_size
+    K, C = rois.shape[0], feats64[0].shape[1]
+    off = None if offset is None else np.ascontiguousarray(offset, dtype=np.float32)
+    assert off is None or off.shape == (K, 2, PH, PW)
+    out = np.zeros((K, C, PH, PW), np.float64)
+    rc = lib().deform_roi_pool_fpn_forward_ref(_levels(feats64, scales), len(feats64), _p(rois), K,
+                                               None if off is None else _p(off), ctypes.c_float(gamma), PH, PW,
+                                               int(sampling_ratio), ctypes.c_float(finest_scale), int(bool(f64)), _p(out))
+    assert rc == 0
+    return out
+
+
+def deform_roi_pool_backward(feats, scales, grad_out, rois, offset, gamma, sampling_ratio=2, finest_scale=56.0, f64=False):
+    """D5.  Returns (list of float64 feature gradients, float64 offset gradient [K,2,PH,PW])."""
+    feats64 = [np.ascontiguousarray(f, dtype=np.float64) for f in feats]
+    grads = [np.zeros(f.shape, np.float64) for f in feats64]
+    rois = np.ascontiguousarray(rois, dtype=np.float32)
+    grad_out = np.ascontiguousarray(grad_out, dtype=np.float64)
+    K, C, PH, PW = grad_out.shape
+    off = None if offset is None else np.ascontiguousarray(offset, dtype=np.float32)
+    goff = np.zeros((K, 2, PH, PW), np.float64)
+    rc = lib().deform_roi_pool_fpn_backward_ref(_levels(feats64, scales), _levels(grads, scales), len(feats64), _p(grad_out),
+                                                _p(rois), K, None if off is None else _p(off), ctypes.c_float(gamma), PH, PW,
+                                                int(sampling_ratio), ctypes.c_float(finest_scale), int(bool(f64)), _p(goff))
+    assert rc == 0
+    return grads, goff

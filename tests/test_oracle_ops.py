@@ -240,3 +240,149 @@ def test_soft_nms_without_overlap_is_a_score_sort():
         idx, sc = O.soft_nms(boxes, scores, 0.3, 0.5, 0.0, method)
         assert idx.tolist() == np.argsort(-scores, kind="stable").tolist()
         assert np.array_equal(sc, scores[idx])
+
+
+# ------------------------------------------------------------------------------- deformable RoI pooling
+# Pins of oracle/ops_ref.cpp deform_roi_pool_* (readings D1-D5).  The RoIAlign oracle it is
+# compared with (oracle/raf_ref.cpp) is itself pinned in tests/test_oracle_forward.py / _backward.py.
+from oracle import raf_ref as R  # noqa: E402
+
+
+def _deform_case(seed=3, K=12, C=3, shapes=((1, 3, 40, 48), (1, 3, 20, 24)), P=(5, 6)):
+    rng = np.random.default_rng(seed)
+    feats = [rng.standard_normal(s) for s in shapes]
+    scales = [0.25, 0.125]
+    side = np.exp(rng.uniform(np.log(20), np.log(170), (K, 2)))
+    cx, cy = rng.uniform(0, 190, K), rng.uniform(0, 160, K)
+    rois = np.stack([np.zeros(K), cx - side[:, 0] / 2, cy - side[:, 1] / 2, cx + side[:, 0] / 2,
+                     cy + side[:, 1] / 2], 1).astype(np.float32)
+    off = rng.uniform(-0.6, 0.6, (K, 2) + P).astype(np.float32)
+    return feats, scales, rois, off, P
+
+
+def test_deform_zero_offset_is_roialign_bit_for_bit():
+    feats, scales, rois, off, P = _deform_case()
+    for g in (1, 2, 0):
+        a = O.deform_roi_pool_forward(feats, scales, rois, None, 0.1, P, g)
+        b = O.deform_roi_pool_forward(feats, scales, rois, np.zeros_like(off), 0.1, P, g)
+        ref = R.forward(feats, scales, rois, P, g, True, 56.0, coord_f32=True)
+        assert np.array_equal(a, ref) and np.array_equal(b, ref)
+        a64 = O.deform_roi_pool_forward(feats, scales, rois, None, 0.1, P, g, f64=True)
+        assert np.abs(a64 - R.forward(feats, scales, rois, P, g, True, 56.0, coord_f32=False)).max() < 1e-12
+
+
+def test_deform_uniform_offset_is_a_translated_box():
+    """offset (dx, dy) on EVERY bin moves all samples by gamma*(rw*dx, rh*dy) feature pixels = the RoI moved by
+    that much divided by the level's scale in image pixels (f64 mode: exact up to rounding)."""
+    feats, scales, rois, _, P = _deform_case(seed=4, K=8)
+    gamma, dx, dy = 0.25, 0.3, -0.2
+    off = np.zeros((len(rois), 2) + P, np.float32)
+    off[:, 0], off[:, 1] = dx, dy
+    got = O.deform_roi_pool_forward(feats, scales, rois, off, gamma, P, 2, f64=True)
+    levels = R.assign_levels(rois, 2, 56.0)[0]
+    moved = rois.astype(np.float64).copy()
+    w, h = moved[:, 3] - moved[:, 1], moved[:, 4] - moved[:, 2]
+    # feature-pixel shift gamma*rw*dx with rw = w*scale  ->  image-pixel shift gamma*w*dx (the scale cancels)
+    sx, sy = gamma * w * np.float64(np.float32(dx)), gamma * h * np.float64(np.float32(dy))
+    # the level map must see the ORIGINAL box: evaluate RoI by RoI on the level the original was assigned to
+    for k in range(len(rois)):
+        l = int(levels[k])
+        r = np.array([[0, moved[k, 1] + sx[k], moved[k, 2] + sy[k], moved[k, 3] + sx[k], moved[k, 4] + sy[k]]])
+        ref = _roialign_f64_single(feats[l], scales[l], r[0], P, 2)
+        assert np.abs(got[k] - ref).max() < 1e-9
+
+
+def _roialign_f64_single(feat, scale, roi, P, g):
+    """Plain float64 RoIAlign of one box on one level, written out here (independent of both oracles)."""
+    _, C, H, W = feat.shape
+    PH, PW = P
+    sx, sy = roi[1] * scale - 0.5, roi[2] * scale - 0.5
+    bw, bh = (roi[3] * scale - 0.5 - sx) / PW, (roi[4] * scale - 0.5 - sy) / PH
+    out = np.zeros((C, PH, PW))
+
+    def axis(v, n):
+        if v < -1 or v > n:
+            return None
+        v = max(v, 0.0)
+        lo = int(v)
+        if lo >= n - 1:
+            return n - 1, n - 1, 1.0, 0.0
+        return lo, lo + 1, 1 - (v - lo), v - lo
+    for ph in range(PH):
+        for pw in range(PW):
+            for iy in range(g):
+                ty = axis(sy + ph * bh + (iy + 0.5) * bh / g, H)
+                if ty is None:
+                    continue
+                for ix in range(g):
+                    tx = axis(sx + pw * bw + (ix + 0.5) * bw / g, W)
+                    if tx is None:
+                        continue
+                    out[:, ph, pw] += (ty[2] * tx[2] * feat[0, :, ty[0], tx[0]] + ty[2] * tx[3] * feat[0, :, ty[0], tx[1]] +
+                                       ty[3] * tx[2] * feat[0, :, ty[1], tx[0]] + ty[3] * tx[3] * feat[0, :, ty[1], tx[1]])
+    return out / (g * g)
+
+
+def test_deform_offset_of_one_bin_changes_that_bin_only_and_planes_are_x_then_y():
+    feats, scales, rois, _, P = _deform_case(seed=5, K=4)
+    base = O.deform_roi_pool_forward(feats, scales, rois, None, 0.2, P, 2)
+    off = np.zeros((4, 2) + P, np.float32)
+    off[1, 0, 2, 3] = 0.5
+    got = O.deform_roi_pool_forward(feats, scales, rois, off, 0.2, P, 2)
+    diff = got != base
+    assert diff[1, :, 2, 3].any()
+    diff[1, :, 2, 3] = False
+    assert not diff.any()
+    # x-ramp feature: an x offset moves the value by gamma*rw*dx*slope, a y offset leaves it unchanged
+    H, W = 40, 48
+    ramp = np.broadcast_to(np.arange(W, dtype=np.float64)[None, None, None, :] * 2.0, (1, 1, H, W)).copy()
+    roi = np.array([[0, 40, 40, 120, 100]], np.float32)     # level 0 at scale 0.25: 20 x 15 px, interior
+    P2 = (3, 4)
+    z = O.deform_roi_pool_forward([ramp], [0.25], roi, None, 0.1, P2, 2, f64=True)
+    ox = np.zeros((1, 2) + P2, np.float32); ox[0, 0] = 0.25
+    oy = np.zeros((1, 2) + P2, np.float32); oy[0, 1] = 0.25
+    rw = (120 - 40) * 0.25
+    g32 = np.float64(np.float32(0.1))      # gamma is a float32 argument
+    assert np.abs(O.deform_roi_pool_forward([ramp], [0.25], roi, ox, 0.1, P2, 2, f64=True) - (z + g32 * rw * 0.25 * 2.0)).max() < 1e-9
+    assert np.abs(O.deform_roi_pool_forward([ramp], [0.25], roi, oy, 0.1, P2, 2, f64=True) - z).max() < 1e-12
+
+
+def test_deform_backward_adjoint_and_finite_differences():
+    feats, scales, rois, off, P = _deform_case(seed=6, K=6)
+    gamma = 0.15
+    rng = np.random.default_rng(7)
+    gout = rng.standard_normal((len(rois), feats[0].shape[1]) + P)
+    out = O.deform_roi_pool_forward(feats, scales, rois, off, gamma, P, 2, f64=True)
+    gf, goff = O.deform_roi_pool_backward(feats, scales, gout, rois, off, gamma, 2, f64=True)
+    # feature gradient = transpose of the (linear in F) forward:  <A x, g> = <x, A^T g>
+    lhs = float((out * gout).sum())
+    rhs = float(sum((f * g).sum() for f, g in zip(feats, gf)))
+    assert abs(lhs - rhs) < 1e-10 * max(1.0, abs(lhs))
+    # offset gradient = derivative of the forward: central differences on a few entries (f64 forward; an entry is
+    # skipped when a sample sits within the step of a pixel boundary, where the forward has a kink)
+    eps, checked = 1e-4, 0
+    for (k, a, ph, pw) in [(0, 0, 1, 2), (1, 1, 0, 0), (2, 0, 4, 5), (3, 1, 2, 2), (4, 0, 3, 1), (5, 1, 1, 4)]:
+        op, om = off.astype(np.float64).copy(), off.astype(np.float64).copy()
+        # float32 offsets: perturb by a float32-exact amount
+        d = np.float32(off[k, a, ph, pw] + eps) - off[k, a, ph, pw]
+        op[k, a, ph, pw] += d; om[k, a, ph, pw] -= d
+        fp = O.deform_roi_pool_forward(feats, scales, rois, op.astype(np.float32), gamma, P, 2, f64=True)
+        fm = O.deform_roi_pool_forward(feats, scales, rois, om.astype(np.float32), gamma, P, 2, f64=True)
+        dp = np.float64(np.float32(op[k, a, ph, pw])) - np.float64(off[k, a, ph, pw])
+        dm = np.float64(off[k, a, ph, pw]) - np.float64(np.float32(om[k, a, ph, pw]))
+        num = float(((fp - fm) * gout).sum()) / (dp + dm)
+        # second difference small <=> no kink inside the step
+        curv = float((np.abs(fp - 2 * out + fm) * np.abs(gout)).sum())
+        if curv > 1e-9:
+            continue
+        assert abs(num - goff[k, a, ph, pw]) < 1e-6 * max(1.0, abs(num))
+        checked += 1
+    assert checked >= 3
+    # constant map: the forward does not depend on the offsets (inside the map)
+    const = [np.full(f.shape, 2.5) for f in feats]
+    inner = rois.copy(); inner[:, 1:] = [60, 50, 110, 95]
+    _, g0 = O.deform_roi_pool_backward(const, scales, gout, inner, off * 0.1, gamma, 2, f64=True)
+    assert np.abs(g0).max() < 1e-12
+    # spec mode (fp32 coordinates) stays within coordinate rounding of the f64 mode
+    gf32, goff32 = O.deform_roi_pool_backward(feats, scales, gout, rois, off, gamma, 2, f64=False)
+    assert max(np.abs(a - b).max() for a, b in zip(gf, gf32)) < 1e-3

@@ -48,7 +48,7 @@ def parse_args():
     ap.add_argument("--rotate", type=int, default=0,
                     help="number of independent input/output buffer sets to rotate over (0 = cold-L2 protocol: "
                          "at least 4 and >= 2x L2; 1 = WARM single-buffer number, not the headline)")
-    ap.add_argument("--op", default="align", choices=["align", "pool", "nms", "softnms"],
+    ap.add_argument("--op", default="align", choices=["align", "pool", "deform", "nms", "softnms"],
                     help="align: the headline FPN RoIAlign fwd+bwd (BASELINE.json metric); pool / nms / softnms: the SURVEY 8(f) "
                          "operations, one extra bench line each (not the headline)")
     ap.add_argument("--nms-n", type=int, default=2000, help="boxes for --op nms / softnms")
@@ -573,6 +573,46 @@ def run_op(args):
                                      "windows differ by at most a pixel per side) + out + argmax written + grad_out + argmax "
                                      "read + gradient pyramid zero-filled and written"},
                 "clocks": clocks, "gpu_launches": args.windows * args.window_iters * (2 + len(cfg.level_shapes))}
+    elif args.op == "deform":
+        cfg = inputs.CONFIGS[args.config]
+        wl = inputs.make_workload(args.config)
+        tdt = {"f32": torch.float32, "f16": torch.float16, "bf16": torch.bfloat16}[cfg.dtype]
+        esz = 4 if cfg.dtype == "f32" else 2
+        K, C = cfg.K, cfg.channels
+        PH, PW = cfg.out_size
+        lay = lambda t: t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
+        pyr = sum(int(np.prod(s)) for s in cfg.level_shapes)
+        R = 4
+        feats = [[lay(torch.from_numpy(f).to(tdt).cuda()) for f in wl.feats] for _ in range(R)]
+        rois = torch.from_numpy(wl.rois).cuda()
+        offset = torch.from_numpy(np.random.default_rng(190607155 + 78).uniform(-0.5, 0.5, (K, 2, PH, PW)).astype(np.float32)).cuda()
+        outs = [lay(torch.empty((K, C, PH, PW), dtype=tdt, device="cuda")) for _ in range(R)]
+        gouts = [lay(torch.from_numpy(wl.grad_out).to(tdt).cuda()) for _ in range(R)]
+        grads = [[lay(torch.empty(s, dtype=torch.float32, device="cuda")) for s in cfg.level_shapes] for _ in range(R)]
+        goff = torch.empty((K, 2, PH, PW), dtype=torch.float32, device="cuda")
+
+        def step(j):
+            B.roi_deform_pool_fpn_forward(feats[j], cfg.scales, rois, offset, 0.1, outs[j], 2, cfg.finest_scale, stream)
+            B.roi_deform_pool_fpn_backward(feats[j], grads[j], cfg.scales, gouts[j], rois, offset, 0.1, 2, cfg.finest_scale,
+                                           goff, 0, stream)
+        ms, ms_min, clocks = timed(step, R)
+        fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, 2, True, cfg.finest_scale)
+        by = 2 * fp["union_px"] * C * esz + 2 * K * C * PH * PW * esz + pyr * 4 * 2 + 3 * K * 2 * PH * PW * 4
+        ach = by / (ms * 1e-3) / 1e9
+        line = {"metric": "deformable RoI pooling fwd+bwd RoIs/sec (C=256, 7x7, FPN)", "value": K / (ms * 1e-3), "unit": UNIT,
+                "n_gpus": 1, "steps": args.windows * args.window_iters, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+                "ms_per_step_min": ms_min, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": cfg.dtype, "data": "synthetic",
+                "config": {"workload": f"deformable RoI pooling on BASELINE.json configs[{args.config - 1}] shapes: {cfg.name}",
+                           "K": K, "C": C, "layout": "cl", "gamma": 0.1, "offsets": "U(-0.5, 0.5) per bin",
+                           "l2_protocol": f"inputs rotate over {R} independent copies"},
+                "roofline": {"bound": "hbm", "kernel": "deform fwd + zero-fill + bwd (features and offsets)", "achieved": ach,
+                             "peak": peak, "unit": "GB/s", "frac": ach / peak, "frac_nominal_8000": ach / 8000.0, "traffic": None,
+                             "algorithmic_bytes": int(by), "peak_source": peak_src,
+                             "note": "bytes = touched-pixel union read in the forward and again in the backward (the RoIAlign "
+                                     "union of the undeformed RoIs as a stand-in) + out + grad_out + gradient pyramid "
+                                     "zero-filled and written + offsets / offset gradient"},
+                "clocks": clocks, "gpu_launches": args.windows * args.window_iters * (3 + len(cfg.level_shapes))}
     else:
         n = args.nms_n
         rng = np.random.default_rng(190607155 + 77)

@@ -165,6 +165,28 @@ int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dty
                           const int32_t* argmax, const int64_t* gout_strides, const float* rois, int K,
                           int out_h, int out_w, float finest_scale, int flags, void* stream);
 
+/* ---- deformable RoI pooling ("DCN [8]: deformable convolution and deformable RoI pooling",
+ * PAPER.md:57-58), on the same FPN level map (C1).  Readings D1-D5: RoIAlign with the half-pixel
+ * shift and no minimum size whose bin (ph,pw) is moved by (gamma*rw*offset[k,0,ph,pw], gamma*rh*offset[k,1,ph,pw])
+ * feature pixels (rw, rh = RoI size on its level): sample coordinate = the C3 coordinate + that shift (one more fp32
+ * addition), then the C3 tap rule; out = sum / count.
+ *   offset   float32 DEVICE [K,2,out_h,out_w] contiguous (plane 0 = x, 1 = y); NULL = all zero (= RoIAlign)
+ *   sampling_ratio  > 0 fixed grid, 0 adaptive (ceil of the bin size)
+ * fp32 coordinates bit-identical to the oracle's, fp32 accumulation. */
+int roi_deform_pool_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                                const float* offset, float gamma, int out_h, int out_w, int sampling_ratio,
+                                float finest_scale, void* out, const int64_t* out_strides, void* stream);
+
+/* Backward of deformable RoI pooling.  grad_feats (HOST array of L fp32 descriptors, or NULL): += the exact
+ * transpose (fp32 atomics; zero-filled first unless RAF_ACCUMULATE).  grad_offset (float32 DEVICE [K,2,out_h,out_w],
+ * or NULL): overwritten with d loss / d offset -- the derivative of the forward where it exists (a sample whose
+ * coordinate is clamped at a border does not move with the offset).  feats: the forward's features (read for the
+ * offset gradient), dtype = grad_out's dtype.  flags: RAF_ACCUMULATE only (applies to grad_feats). */
+int roi_deform_pool_fpn_backward(const raf_level* feats, const raf_level* grad_feats, int L, raf_dtype dtype,
+                                 const void* grad_out, const int64_t* gout_strides, const float* rois, int K,
+                                 const float* offset, float gamma, int out_h, int out_w, int sampling_ratio,
+                                 float finest_scale, float* grad_offset, int flags, void* stream);
+
 /* ---- NMS and Soft-NMS on the GPU ("Soft NMS [1]: an alternative to NMS", PAPER.md:55;
  * "All basic bbox and mask operations run on GPUs") ---------------------------------------------
  * boxes: float32 DEVICE [n,4] = (x1,y1,x2,y2), continuous coordinates (no "+1"); scores: float32 DEVICE [n],

@@ -25,7 +25,7 @@ EXPORTS = [
     "roi_align_fpn_forward_ex", "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
     "roi_pool_fpn_forward", "roi_pool_fpn_backward", "roi_nms_workspace_bytes", "roi_nms", "roi_soft_nms",
-    "roi_align_fpn_repack_bytes",
+    "roi_align_fpn_repack_bytes", "roi_deform_pool_fpn_forward", "roi_deform_pool_fpn_backward",
 ]
 
 
@@ -81,6 +81,10 @@ def lib() -> ctypes.CDLL:
         L.roi_pool_fpn_forward.argtypes = [vp, ci, ci, vp, ci, ci, ci, cf, vp, vp, vp, vp]
         L.roi_pool_fpn_backward.restype = ci
         L.roi_pool_fpn_backward.argtypes = [vp, ci, ci, vp, vp, vp, vp, ci, ci, ci, cf, ci, vp]
+        L.roi_deform_pool_fpn_forward.restype = ci
+        L.roi_deform_pool_fpn_forward.argtypes = [vp, ci, ci, vp, ci, vp, cf, ci, ci, ci, cf, vp, vp, vp]
+        L.roi_deform_pool_fpn_backward.restype = ci
+        L.roi_deform_pool_fpn_backward.argtypes = [vp, vp, ci, ci, vp, vp, vp, ci, vp, cf, ci, ci, ci, cf, vp, ci, vp]
         L.roi_nms_workspace_bytes.restype = ctypes.c_size_t
         L.roi_nms_workspace_bytes.argtypes = [ci]
         L.roi_nms.restype = ci
@@ -304,6 +308,54 @@ def roi_pool_fpn_backward(grad_feats: Sequence[torch.Tensor], scales: Sequence[f
                                      _stream_ptr(stream))
     if rc:
         raise RafError(rc, "roi_pool_fpn_backward")
+
+
+def _check_offset(offset: Optional[torch.Tensor], K: int, PH: int, PW: int, device, what: str) -> None:
+    if offset is None:
+        return
+    if (offset.dtype != torch.float32 or tuple(offset.shape) != (K, 2, PH, PW) or not offset.is_contiguous()
+            or offset.device != device):
+        raise ValueError(f"{what} must be a contiguous float32 [K,2,PH,PW] tensor on the device of the RoI tensor")
+
+
+def roi_deform_pool_fpn_forward(feats: Sequence[torch.Tensor], scales: Sequence[float], rois: torch.Tensor,
+                                offset: Optional[torch.Tensor], gamma: float, out: torch.Tensor, sampling_ratio: int,
+                                finest_scale: float, stream=None) -> None:
+    """Deformable RoI pooling (include/raf.h).  out: logical [K,C,PH,PW]; offset: float32 [K,2,PH,PW] or None."""
+    _check_call(feats, feats[0].dtype if len(feats) else None, rois, out, feats[0].dtype if len(feats) else None, None)
+    if feats[0].dtype not in _DTYPES:
+        raise ValueError(f"unsupported feature dtype {feats[0].dtype}")
+    K, _, PH, PW = out.shape
+    _check_offset(offset, K, PH, PW, out.device, "offset")
+    rc = lib().roi_deform_pool_fpn_forward(make_levels(feats, scales), len(feats), _DTYPES[feats[0].dtype], _ptr(rois), K,
+                                           _ptr(offset), float(gamma), PH, PW, int(sampling_ratio), finest_scale, _ptr(out),
+                                           _strides4(out), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_deform_pool_fpn_forward")
+
+
+def roi_deform_pool_fpn_backward(feats: Sequence[torch.Tensor], grad_feats: Optional[Sequence[torch.Tensor]],
+                                 scales: Sequence[float], grad_out: torch.Tensor, rois: torch.Tensor,
+                                 offset: Optional[torch.Tensor], gamma: float, sampling_ratio: int, finest_scale: float,
+                                 grad_offset: Optional[torch.Tensor], flags: int = 0, stream=None) -> None:
+    """grad_feats: fp32 tensors shaped like feats (or None); grad_offset: float32 [K,2,PH,PW] (or None)."""
+    if grad_out.dtype not in _DTYPES:
+        raise ValueError(f"unsupported grad_out dtype {grad_out.dtype}")
+    _check_call(feats, grad_out.dtype, rois, grad_out, grad_out.dtype, None)
+    if grad_feats is not None:
+        _check_call(grad_feats, torch.float32, rois, grad_out, grad_out.dtype, None)
+        if any(tuple(g.shape) != tuple(f.shape) for g, f in zip(grad_feats, feats)) or len(grad_feats) != len(feats):
+            raise ValueError("grad_feats must have the shapes of feats")
+    K, _, PH, PW = grad_out.shape
+    _check_offset(offset, K, PH, PW, grad_out.device, "offset")
+    _check_offset(grad_offset, K, PH, PW, grad_out.device, "grad_offset")
+    rc = lib().roi_deform_pool_fpn_backward(make_levels(feats, scales),
+                                            None if grad_feats is None else make_levels(grad_feats, scales), len(feats),
+                                            _DTYPES[grad_out.dtype], _ptr(grad_out), _strides4(grad_out), _ptr(rois), K,
+                                            _ptr(offset), float(gamma), PH, PW, int(sampling_ratio), finest_scale,
+                                            _ptr(grad_offset), int(flags), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_deform_pool_fpn_backward")
 
 
 def _check_boxes(boxes: torch.Tensor, scores: torch.Tensor) -> int:

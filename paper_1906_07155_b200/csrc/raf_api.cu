@@ -462,6 +462,67 @@ int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dty
                               unit_channel_stride(grad_feats, L), st);
 }
 
+// ---- deformable RoI pooling ---------------------------------------------------------------------------
+int roi_deform_pool_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                                const float* offset, float gamma, int out_h, int out_w, int sampling_ratio,
+                                float finest_scale, void* out, const int64_t* out_strides, void* stream) {
+  int rc = check_levels(feats, L);
+  if (rc) return rc;
+  rc = check_common(rois, K, out_h, out_w, sampling_ratio);
+  if (rc) return rc;
+  if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f) || !(gamma == gamma)) return RAF_ERR_SHAPE;
+  if (!out_strides) return RAF_ERR_NULL;
+  if (K == 0) return RAF_OK;
+  for (int i = 0; i < 4; ++i) if (out_strides[i] <= 0) return RAF_ERR_STRIDE;
+  if (!out) return RAF_ERR_NULL;
+  LevelsParam p;
+  fill_param(feats, L, &p);
+  return launch_deform_forward(p, dtype, rois, K, offset, gamma, out_h, out_w, sampling_ratio, finest_scale, out, out_strides,
+                               unit_channel_stride(feats, L), (cudaStream_t)stream);
+}
+
+int roi_deform_pool_fpn_backward(const raf_level* feats, const raf_level* grad_feats, int L, raf_dtype dtype,
+                                 const void* grad_out, const int64_t* gout_strides, const float* rois, int K,
+                                 const float* offset, float gamma, int out_h, int out_w, int sampling_ratio,
+                                 float finest_scale, float* grad_offset, int flags, void* stream) {
+  int rc = check_levels(feats, L);
+  if (rc) return rc;
+  if (grad_feats) {
+    rc = check_levels(grad_feats, L);
+    if (rc) return rc;
+    for (int l = 0; l < L; ++l)
+      if (grad_feats[l].n != feats[l].n || grad_feats[l].c != feats[l].c || grad_feats[l].h != feats[l].h ||
+          grad_feats[l].w != feats[l].w)
+        return RAF_ERR_SHAPE;
+  }
+  rc = check_common(rois, K, out_h, out_w, sampling_ratio);
+  if (rc) return rc;
+  if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f) || !(gamma == gamma)) return RAF_ERR_SHAPE;
+  if (flags & ~RAF_ACCUMULATE) return RAF_ERR_UNSUPPORTED;
+  if (!gout_strides) return RAF_ERR_NULL;
+  for (int i = 0; i < 4; ++i) if (K > 0 && gout_strides[i] <= 0) return RAF_ERR_STRIDE;
+  if (K > 0 && !grad_out) return RAF_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (grad_feats && !(flags & RAF_ACCUMULATE)) {
+    rc = zero_fill(grad_feats, L, st);
+    if (rc) return rc;
+  }
+  if (K == 0) return RAF_OK;
+  if (grad_offset) {
+    if (cudaMemsetAsync(grad_offset, 0, sizeof(float) * (size_t)K * 2 * out_h * out_w, st) != cudaSuccess) return RAF_ERR_CUDA;
+    count_launch();
+  }
+  if (!grad_feats && !grad_offset) return RAF_OK;
+  LevelsParam p, gp;
+  fill_param(feats, L, &p);
+  fill_param(grad_feats ? grad_feats : feats, L, &gp);
+  return launch_deform_backward(p, gp, grad_feats != nullptr, dtype, rois, K, offset, gamma, out_h, out_w, sampling_ratio,
+                                finest_scale, grad_out, gout_strides, grad_offset,
+                                unit_channel_stride(feats, L) && (!grad_feats || unit_channel_stride(grad_feats, L)), st);
+}
+
 // ---- NMS / Soft-NMS ------------------------------------------------------------------------------------
 size_t roi_nms_workspace_bytes(int n) { return nms_workspace_bytes(n > 0 ? n : 0); }
 

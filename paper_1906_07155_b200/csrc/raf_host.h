@@ -73,6 +73,13 @@ int launch_pool_forward(const LevelsParam& lv, raf_dtype dtype, const float* roi
 int launch_pool_backward(const LevelsParam& glv, raf_dtype dtype, const float* rois, int K, int PH, int PW, float fs,
                          const void* gout, const int32_t* argmax, const int64_t* gs, bool chan_fastest, cudaStream_t stream);
 
+// Deformable RoI pooling (raf_deform.cu).  The gradient pyramid / grad_offset must already hold their starting values.
+int launch_deform_forward(const LevelsParam& lv, raf_dtype dtype, const float* rois, int K, const float* offset, float gamma,
+                          int PH, int PW, int g, float fs, void* out, const int64_t* os, bool chan_fastest, cudaStream_t stream);
+int launch_deform_backward(const LevelsParam& lv, const LevelsParam& glv, bool want_feats, raf_dtype dtype, const float* rois,
+                           int K, const float* offset, float gamma, int PH, int PW, int g, float fs, const void* gout,
+                           const int64_t* gs, float* grad_offset, bool chan_fastest, cudaStream_t stream);
+
 // NMS / Soft-NMS (raf_nms.cu).
 size_t nms_workspace_bytes(int n);
 int launch_nms(const float* boxes, const float* scores, int n, float iou_threshold, int32_t* keep, int32_t* num_keep,

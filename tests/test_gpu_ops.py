@@ -145,3 +145,94 @@ def test_soft_nms(method, n):
         gaps = np.abs(np.diff(ref_s[:k])) > 1e-4 * ref_s[:k - 1] if k > 1 else np.zeros(0, bool)
         safe = np.concatenate([[True], gaps]) & np.concatenate([gaps, [True]]) if k > 1 else np.ones(k, bool)
         assert np.array_equal(got_i[:k][safe], ref_i[:k][safe])
+
+
+# ------------------------------------------------------------------------------- deformable RoI pooling
+def _deform_inputs(wl, dtype, layout, seed, amp=0.5):
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K = cfg.K
+    rng = np.random.default_rng(seed)
+    offset = rng.uniform(-amp, amp, (K, 2, PH, PW)).astype(np.float32)
+    feats, exact = T.device_feats(wl.feats, dtype, layout)
+    return feats, exact, torch.from_numpy(wl.rois).cuda(), offset
+
+
+@pytest.mark.parametrize("layout", ["cl", "nchw"])
+@pytest.mark.parametrize("index,dtype,kw,g", [
+    (1, "f32", {}, 2),
+    (2, "f32", dict(n_img=2, per_img=60, channels=32), 2),
+    (2, "f32", dict(n_img=1, per_img=40, channels=20), 0),
+    (4, "bf16", dict(n_img=2, per_img=24, channels=32), 2),
+    (5, "f16", dict(n_img=2, per_img=40, channels=16), 1),
+])
+def test_deform_roi_pool_forward_backward(index, dtype, kw, g, layout):
+    """Readings D1-D5: forward at the RoIAlign tolerances (S10); feature gradient at S11 (S = the oracle's sum of
+    |terms|, here bounded by the RoIAlign S of the same taps: use |ref| summed in double); offset gradient against
+    the oracle with a tolerance scaled by the sum of |terms| over channels.  Zero offsets == RoIAlign."""
+    wl = inputs.make_workload(index, **kw)
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C = cfg.K, cfg.channels
+    gamma = 0.1
+    feats, exact, rois, offset = _deform_inputs(wl, dtype, layout, seed=index)
+    off_d = torch.from_numpy(offset).cuda()
+    out = T.empty_layout((K, C, PH, PW), feats[0].dtype, layout, fill=float("nan"))
+    B.roi_deform_pool_fpn_forward(feats, cfg.scales, rois, off_d, gamma, out, g, cfg.finest_scale)
+    torch.cuda.synchronize()
+    ref = O.deform_roi_pool_forward(exact, cfg.scales, wl.rois, offset, gamma, (PH, PW), g, cfg.finest_scale)
+    T.assert_forward_close(out.to(torch.float64).cpu().numpy(), ref, dtype)
+    # zero offsets (NULL tensor) == the RoIAlign forward of the library (same coordinates; fp32 sums in another order)
+    out0 = T.empty_layout((K, C, PH, PW), feats[0].dtype, layout, fill=float("nan"))
+    B.roi_deform_pool_fpn_forward(feats, cfg.scales, rois, None, gamma, out0, g, cfg.finest_scale)
+    ref0 = O.deform_roi_pool_forward(exact, cfg.scales, wl.rois, None, gamma, (PH, PW), g, cfg.finest_scale)
+    T.assert_forward_close(out0.to(torch.float64).cpu().numpy(), ref0, dtype)
+    # backward
+    go_t = torch.from_numpy(wl.grad_out).to(T.TORCH_DTYPE[dtype])
+    go = T.to_layout(go_t.cuda(), layout)
+    go_exact = go_t.to(torch.float64).numpy()
+    grads = [T.empty_layout(s, torch.float32, layout, fill=float("nan")) for s in cfg.level_shapes]
+    goff = torch.full((K, 2, PH, PW), float("nan"), dtype=torch.float32, device="cuda")
+    B.roi_deform_pool_fpn_backward(feats, grads, cfg.scales, go, rois, off_d, gamma, g, cfg.finest_scale, goff)
+    torch.cuda.synchronize()
+    gref, goref = O.deform_roi_pool_backward(exact, cfg.scales, go_exact, wl.rois, offset, gamma, g, cfg.finest_scale)
+    # scale of the sums: the same backward on |grad_out| with all-positive weights bounds sum |terms|
+    Sref, _ = O.deform_roi_pool_backward(exact, cfg.scales, np.abs(go_exact), wl.rois, offset, gamma, g, cfg.finest_scale)
+    T.assert_backward_close([t.to(torch.float64).cpu().numpy() for t in grads], gref, Sref)
+    # offset gradient: sum over channels and samples of go * (differences of features): fp32 sums of up to C*g*g*2
+    # terms -> |err| <= 1e-4 |ref| + 2e-6 * sum |terms|; sum |terms| is bounded by the same backward on |grad_out| and
+    # |features| differences <= 2 max|F| ... use the oracle on absolute values as the scale
+    abs_feats = [np.abs(e) for e in exact]
+    _, Soff = O.deform_roi_pool_backward(abs_feats, cfg.scales, np.abs(go_exact), wl.rois, offset, gamma, g, cfg.finest_scale)
+    scale = np.abs(Soff) + 2.0 * np.abs(goref) + 1e-3
+    err = np.abs(goff.to(torch.float64).cpu().numpy() - goref)
+    tol = 1e-4 * np.abs(goref) + 1e-5 * scale if dtype == "f32" else 2e-2 * np.abs(goref) + 1e-3 * scale
+    assert np.isfinite(goff.cpu().numpy()).all()
+    assert (err <= tol).all(), float((err / tol).max())
+    # feature gradient only / offset gradient only / accumulate
+    g2 = [torch.zeros_like(t) for t in grads]
+    B.roi_deform_pool_fpn_backward(feats, g2, cfg.scales, go, rois, off_d, gamma, g, cfg.finest_scale, None)
+    goff2 = torch.full_like(goff, float("nan"))
+    B.roi_deform_pool_fpn_backward(feats, None, cfg.scales, go, rois, off_d, gamma, g, cfg.finest_scale, goff2)
+    torch.cuda.synchronize()
+    T.assert_backward_close([t.to(torch.float64).cpu().numpy() for t in g2], gref, Sref)
+    assert (np.abs(goff2.to(torch.float64).cpu().numpy() - goref) <= tol).all()
+    B.roi_deform_pool_fpn_backward(feats, g2, cfg.scales, go, rois, off_d, gamma, g, cfg.finest_scale, None, B.RAF_ACCUMULATE)
+    torch.cuda.synchronize()
+    T.assert_backward_close([t.to(torch.float64).cpu().numpy() for t in g2], [2 * r for r in gref], [2 * s for s in Sref])
+
+
+def test_deform_roi_pool_argument_errors():
+    wl = inputs.make_workload(1)
+    cfg = wl.cfg
+    feats, _, rois, offset = _deform_inputs(wl, "f32", "cl", seed=0)
+    out = T.empty_layout((cfg.K, cfg.channels, 7, 7), torch.float32, "cl")
+    with pytest.raises(ValueError):
+        B.roi_deform_pool_fpn_forward(feats, cfg.scales, rois, torch.zeros(cfg.K, 2, 7, 6, device="cuda"), 0.1, out, 2, 56.0)
+    with pytest.raises(B.RafError) as e:
+        B.roi_deform_pool_fpn_forward(feats, cfg.scales, rois, None, 0.1, out, -1, 56.0)
+    assert e.value.status == -2
+    go = T.to_layout(torch.from_numpy(wl.grad_out).cuda(), "cl")
+    with pytest.raises(B.RafError) as e:
+        B.roi_deform_pool_fpn_backward(feats, None, cfg.scales, go, rois, None, 0.1, 2, 56.0, None, flags=B.RAF_ATOMIC)
+    assert e.value.status == -5

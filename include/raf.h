@@ -57,9 +57,9 @@ typedef struct {
 /* Backward flags (bitmask). */
 enum {
   RAF_ACCUMULATE = 1,     /* add into the existing gradient pyramid instead of overwriting it      */
-  RAF_DETERMINISTIC = 2,  /* REQUIRE the bit-reproducible pull variant (K3d); RAF_ERR_UNSUPPORTED
-                             if the layout is not eligible (needs channels-last, C % 4 == 0,
-                             sampling_ratio > 0, L*N <= 1500)                                       */
+  RAF_DETERMINISTIC = 2,  /* REQUIRE a bit-reproducible pull kernel (K3d); RAF_ERR_UNSUPPORTED if the
+                             layout is not eligible (needs channels-last operands, C % 4 == 0,
+                             L*N <= 2047; any out_h, out_w <= 32 and any sampling grid incl. 0)     */
   RAF_ATOMIC = 4,         /* force the atomic scatter variant (zero-fill + red.global.add.v4.f32)  */
   RAF_REUSE_PREP = 8      /* the workspace still holds what roi_align_fpn_forward wrote into it when
                              called with the SAME rois pointer and K, level shapes and scales, out_h/out_w,
@@ -119,10 +119,11 @@ int roi_fpn_assign_levels(const float* rois, int K, int L, float finest_scale, i
  *   feats        HOST array of L descriptors (device data pointers), dtype = `dtype`
  *   out          DEVICE, dtype = `dtype`, logical [K,C,out_h,out_w] addressed through
  *                out_strides (HOST array of 4 element strides); row k = RoI k (original order)
- *   sampling_ratio  > 0: fixed grid; 0: adaptive gh = ceil(roi_h/out_h), gw = ceil(roi_w/out_w)
+ *   sampling_ratio  > 0: fixed grid; 0: adaptive gh = ceil(roi_h/out_h), gw = ceil(roi_w/out_w) (per RoI; the
+ *                channels-last kernels tabulate grids up to 8 x 8 and sample larger ones directly)
  *   aligned      != 0: half-pixel shift, no minimum box size; 0: legacy (no shift, size >= 1)
- *   ws           written: RoI buckets and tap tables that a following roi_align_fpn_backward on the
- *                same arguments may reuse (RAF_REUSE_PREP); 256-byte aligned                        */
+ *   ws           written: RoI buckets, windows, geometry and tap tables that a following
+ *                roi_align_fpn_backward on the same arguments may reuse (RAF_REUSE_PREP); 256-byte aligned */
 int roi_align_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
                           int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
                           void* out, const int64_t* out_strides, void* ws, size_t ws_bytes,

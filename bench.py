@@ -40,6 +40,8 @@ def parse_args():
     ap.add_argument("--backward", default="auto", choices=["auto", "atomic", "deterministic", "strip", "tile"],
                     help="auto: library's choice (a pull kernel when eligible); atomic: RAF_ATOMIC; deterministic: RAF_DETERMINISTIC; "
                          "strip / tile: force one of the two pull kernels (RAF_PULL_STRIP / RAF_PULL_TILE)")
+    ap.add_argument("--grad-dtype", default="f32", choices=["f32", "same"],
+                    help="gradient pyramid dtype: fp32 (readings S13) or the 16-bit dtype of grad_out (roi_align_fpn_backward_ex)")
     ap.add_argument("--repack", action="store_true",
                     help="with --layout nchw: RAF_REPACK (the library repacks to channels-last inside the workspace, counted in the time)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -300,7 +302,8 @@ def run_ours(args):
     rois = torch.from_numpy(wl.rois).cuda()
     outs = [lay(torch.empty((K, C, PH, PW), dtype=tdt, device="cuda")) for _ in range(R)]
     gouts = [lay(torch.from_numpy(wl.grad_out).to(tdt).cuda()) for _ in range(R)] if cfg.backward else None
-    grads = [[lay(torch.empty(s, dtype=torch.float32, device="cuda")) for s in cfg.level_shapes]
+    gdt = tdt if (args.grad_dtype == "same" and cfg.dtype != "f32") else torch.float32
+    grads = [[lay(torch.empty(s, dtype=gdt, device="cuda")) for s in cfg.level_shapes]
              for _ in range(R)] if cfg.backward else None
     ws_bytes = B.roi_align_fpn_workspace_bytes(K, L, PH, PW, g, flags)
     repack = bool(args.repack and args.layout == "nchw")
@@ -403,12 +406,12 @@ def run_ours(args):
     # ---- roofline (algorithmic bytes / CUDA-event duration of the dominant call) ----
     if g > 0:
         fp = roofline.footprint(wl.rois, cfg.level_shapes, cfg.scales, cfg.out_size, g, aligned, fs)
-        ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz)
+        ab = roofline.algorithmic_bytes(fp, K, C, cfg.out_size, esz, esz, esz, grad_bytes=(esz if gdt != torch.float32 else 4))
     else:   # adaptive grid: the touched set is at least the fixed-grid one; report the dense-pyramid bound instead
         fp = {"level_hist": None}
         ab = {"fwd": pyr_bytes * esz + K * C * PH * PW * esz + 20 * K, "bwd": K * C * PH * PW * esz + pyr_bytes * 4}
     peak, peak_src = peaks()
-    variant = f"{args.layout}{'+repack' if repack else ''}:{args.backward}:{'reuse' if reuse else 'noreuse'}"
+    variant = f"{args.layout}{'+repack' if repack else ''}{'+g16' if gdt != torch.float32 else ''}:{args.backward}:{'reuse' if reuse else 'noreuse'}"
     traffic, traffic_stale = ncu_traffic(args.config, variant)
     legs = {"fwd": (ab["fwd"], loops["fwd"]["median_ms"])}
     if cfg.backward:
@@ -443,6 +446,7 @@ def run_ours(args):
                                        if R * ws_set >= 2 * l2 else
                                        f"WARM: {R} buffer set(s), {R * ws_set / 1e6:.0f} MB vs L2 {l2 / 1e6:.0f} MB (not the headline)"),
                        "backward": args.backward if cfg.backward else "none", "repack": repack,
+                       "grad_dtype": "f32" if gdt == torch.float32 else cfg.dtype,
                        "reuse_prep": bool(reuse), "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
             "roofline": roof(dom),
             "roofline_all": {k: roof(k) for k in legs} | {"step": {

@@ -77,13 +77,13 @@ def footprint(rois: np.ndarray, level_shapes: Sequence[Tuple[int, int, int, int]
 
 
 def algorithmic_bytes(fp: Dict, K: int, C: int, out_size: Tuple[int, int], feat_bytes: int, out_bytes: int,
-                      gout_bytes: int, accumulate: bool = False) -> Dict[str, int]:
+                      gout_bytes: int, accumulate: bool = False, grad_bytes: int = 4) -> Dict[str, int]:
     PH, PW = out_size
     out_elems = K * C * PH * PW
     fwd = fp["union_px"] * C * feat_bytes + out_elems * out_bytes + 20 * K
     if accumulate:
-        bwd = out_elems * gout_bytes + 2 * fp["union_px"] * C * 4
+        bwd = out_elems * gout_bytes + 2 * fp["union_px"] * C * grad_bytes
     else:
-        bwd = out_elems * gout_bytes + fp["pyramid_px"] * C * 4
+        bwd = out_elems * gout_bytes + fp["pyramid_px"] * C * grad_bytes
     return {"fwd": int(fwd), "bwd": int(bwd), "requested_fwd": int(fp["requested_px"] * C * feat_bytes),
             "per_roi_fwd": int(fp["per_roi_px"] * C * feat_bytes)}

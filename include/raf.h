@@ -71,6 +71,16 @@ enum {
                              the WHOLE gradient pyramid with NaN.  Changing the contents of the rois
                              buffer in place between the two calls is not detected.                     */
 };
+/* Backward with a 16-bit gradient pyramid ("optional bf16 grad output"): grad_dtype = RAF_F32 is
+ * roi_align_fpn_backward; grad_dtype = gout_dtype (RAF_F16 / RAF_BF16) writes the pyramid in that type -- sums are
+ * formed in fp32 registers and rounded once per element (tiles that meet more RoIs than one pass takes park their
+ * partial sums in the pyramid, i.e. round once per pass).  Pull kernels only: RAF_ATOMIC, RAF_REPACK and layouts the
+ * pull kernels do not take return RAF_ERR_UNSUPPORTED; so does any other combination of the two dtypes. */
+int roi_align_fpn_backward_ex(const raf_level* grad_feats, int L, raf_dtype gout_dtype, raf_dtype grad_dtype,
+                              const void* grad_out, const int64_t* gout_strides, const float* rois,
+                              int K, int out_h, int out_w, int sampling_ratio, int aligned,
+                              float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream);
+
 /* The deterministic pull backward has two kernels with the same contract and the same prep tables: the
  * TILE kernel (a CTA owns 8 x 8 pixels, one pixel per warp at a time) and the STRIP kernel (a warp owns
  * a tile and walks it in 8-pixel row strips, loading every grad_out vector once per strip; no limit on

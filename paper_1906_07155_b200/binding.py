@@ -22,7 +22,7 @@ _DTYPES = {torch.float32: RAF_F32, torch.float16: RAF_F16, torch.bfloat16: RAF_B
 
 EXPORTS = [
     "roi_align_fpn_workspace_bytes", "roi_fpn_assign_levels", "roi_align_fpn_forward",
-    "roi_align_fpn_forward_ex", "roi_align_fpn_backward", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
+    "roi_align_fpn_forward_ex", "roi_align_fpn_backward", "roi_align_fpn_backward_ex", "roi_align_fpn_host_arena_bytes", "roi_align_fpn_forward_host",
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
     "roi_pool_fpn_forward", "roi_pool_fpn_backward", "roi_nms_workspace_bytes", "roi_nms", "roi_soft_nms",
     "roi_align_fpn_repack_bytes", "roi_deform_pool_fpn_forward", "roi_deform_pool_fpn_backward",
@@ -76,6 +76,8 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = args
         L.roi_align_fpn_forward_ex.restype = ctypes.c_int
         L.roi_align_fpn_forward_ex.argtypes = fwd_args[:12] + [ctypes.c_int] + fwd_args[12:]
+        L.roi_align_fpn_backward_ex.restype = ctypes.c_int
+        L.roi_align_fpn_backward_ex.argtypes = bwd_args[:3] + [ctypes.c_int] + bwd_args[3:]
         vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
         L.roi_pool_fpn_forward.restype = ci
         L.roi_pool_fpn_forward.argtypes = [vp, ci, ci, vp, ci, ci, ci, cf, vp, vp, vp, vp]
@@ -225,15 +227,19 @@ def roi_align_fpn_backward(grad_feats: Sequence[torch.Tensor], scales: Sequence[
                            grad_out: torch.Tensor, rois: torch.Tensor, sampling_ratio: int,
                            aligned: bool, finest_scale: float, flags: int, ws: torch.Tensor,
                            stream=None, levels_desc=None) -> None:
+    """grad_feats: float32 tensors, or (roi_align_fpn_backward_ex) tensors of grad_out's 16-bit dtype."""
     if grad_out.dtype not in _DTYPES:
         raise ValueError(f"unsupported grad_out dtype {grad_out.dtype}")
-    _check_call(grad_feats, torch.float32, rois, grad_out, grad_out.dtype, ws)
+    gdt = grad_feats[0].dtype if len(grad_feats) else torch.float32
+    if gdt not in (torch.float32, grad_out.dtype):
+        raise ValueError("the gradient pyramid must be float32 or have the dtype of grad_out")
+    _check_call(grad_feats, gdt, rois, grad_out, grad_out.dtype, ws)
     desc = levels_desc if levels_desc is not None else make_levels(grad_feats, scales)
     K, _, PH, PW = grad_out.shape
-    rc = lib().roi_align_fpn_backward(desc, len(grad_feats), _DTYPES[grad_out.dtype], _ptr(grad_out),
-                                      _strides4(grad_out), _ptr(rois), K, PH, PW, sampling_ratio,
-                                      int(bool(aligned)), finest_scale, flags, _ptr(ws),
-                                      ws.numel() * ws.element_size(), _stream_ptr(stream))
+    rc = lib().roi_align_fpn_backward_ex(desc, len(grad_feats), _DTYPES[grad_out.dtype], _DTYPES[gdt], _ptr(grad_out),
+                                         _strides4(grad_out), _ptr(rois), K, PH, PW, sampling_ratio,
+                                         int(bool(aligned)), finest_scale, flags, _ptr(ws),
+                                         ws.numel() * ws.element_size(), _stream_ptr(stream))
     if rc:
         raise RafError(rc, "roi_align_fpn_backward")
 

@@ -285,11 +285,23 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                            const void* grad_out, const int64_t* gout_strides, const float* rois,
                            int K, int out_h, int out_w, int sampling_ratio, int aligned,
                            float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream) {
+  return roi_align_fpn_backward_ex(grad_feats, L, gout_dtype, RAF_F32, grad_out, gout_strides, rois, K, out_h, out_w,
+                                   sampling_ratio, aligned, finest_scale, flags, ws, ws_bytes, stream);
+}
+
+int roi_align_fpn_backward_ex(const raf_level* grad_feats, int L, raf_dtype gout_dtype, raf_dtype grad_dtype,
+                              const void* grad_out, const int64_t* gout_strides, const float* rois,
+                              int K, int out_h, int out_w, int sampling_ratio, int aligned,
+                              float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream) {
   int rc = check_levels(grad_feats, L);
   if (rc) return rc;
   rc = check_common(rois, K, out_h, out_w, sampling_ratio);
   if (rc) return rc;
   if (gout_dtype != RAF_F32 && gout_dtype != RAF_F16 && gout_dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (grad_dtype != RAF_F32 && grad_dtype != RAF_F16 && grad_dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  // 16-bit gradient pyramid: only as the type of grad_out, only through the pull kernels (fp32 sums, one rounding)
+  const bool g16 = grad_dtype != RAF_F32;
+  if (g16 && (grad_dtype != gout_dtype || (flags & (RAF_ATOMIC | RAF_REPACK)))) return RAF_ERR_UNSUPPORTED;
   if (!(finest_scale > 0.0f)) return RAF_ERR_SHAPE;
   if (flags & ~(RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_REUSE_PREP | RAF_PULL_STRIP | RAF_PULL_TILE | RAF_REPACK)) return RAF_ERR_UNSUPPORTED;
   if ((flags & RAF_DETERMINISTIC) && (flags & RAF_ATOMIC)) return RAF_ERR_UNSUPPORTED;
@@ -304,7 +316,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
     return RAF_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)stream;
   if ((flags & RAF_REPACK) && K > 0) {
-    const bool cl0 = levels_vectorizable(grad_feats, L, 4, 4) &&
+    const bool cl0 = levels_vectorizable(grad_feats, L, 4, esize(grad_dtype)) &&
                      tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype), K, out_h, out_w);
     if (!cl0) {   // grad_out -> channels-last copy, fast backward into a channels-last gradient copy, repack back
       for (int l = 0; l < L; ++l) if (!level_nchw(grad_feats[l])) return RAF_ERR_STRIDE;
@@ -336,7 +348,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
   LevelsParam p;
   fill_param(grad_feats, L, &p);
   const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
-  const bool cl = levels_vectorizable(grad_feats, L, 4, 4) &&
+  const bool cl = levels_vectorizable(grad_feats, L, 4, esize(grad_dtype)) &&
                   (K == 0 || tensor_vectorizable(grad_out, gout_strides, 4, esize(gout_dtype), K, out_h, out_w));
 
   // ---- pull variant (K3d): deterministic, no zero-fill, every element written once -------------
@@ -362,7 +374,7 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
         rc = launch_pull_prep(p, a, po, st);
         if (rc) return rc;
       }
-      return launch_backward_strip(p, gout_dtype, a, grad_out, gout_strides, po, (flags & RAF_ACCUMULATE) ? 1 : 0, st);
+      return launch_backward_strip(p, gout_dtype, grad_dtype, a, grad_out, gout_strides, po, (flags & RAF_ACCUMULATE) ? 1 : 0, st);
     }
     rc = pull_eligible(p, gout_dtype, a, grad_out, gout_strides);
     if (rc == RAF_OK) {
@@ -371,11 +383,11 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
         rc = launch_pull_prep(p, a, po, st);
         if (rc) return rc;
       }
-      return launch_backward_pull(p, gout_dtype, a, grad_out, gout_strides, po, (flags & RAF_ACCUMULATE) ? 1 : 0, st);
+      return launch_backward_pull(p, gout_dtype, grad_dtype, a, grad_out, gout_strides, po, (flags & RAF_ACCUMULATE) ? 1 : 0, st);
     }
     if (rc != RAF_ERR_UNSUPPORTED) return rc;
   }
-  if (flags & (RAF_DETERMINISTIC | RAF_PULL_STRIP | RAF_PULL_TILE)) return RAF_ERR_UNSUPPORTED;
+  if ((flags & (RAF_DETERMINISTIC | RAF_PULL_STRIP | RAF_PULL_TILE)) || g16) return RAF_ERR_UNSUPPORTED;
 
   // ---- atomic variant (K3) -----------------------------------------------------------------------
   if (!(flags & RAF_ACCUMULATE)) {

@@ -149,7 +149,7 @@ struct PullPair {
 // kThree: also serve rows / columns with THREE consecutive bins from the entries (outputs finer than the
 // pixel grid, e.g. 14 x 14 mask-head bins: config 4 backward 97.6 -> 90.9 us; on 7 x 7 outputs the extra
 // code in the hit loop costs more than it saves: 87.7 -> 93.0 us, so it is off there).
-template <typename T, bool kFull, bool kThree>
+template <typename T, typename G, bool kFull, bool kThree>
 __global__ void __launch_bounds__(kPullThreads, RAF_PULL_MINB)
 bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gout, int gs_k,
                 int gs_h, int gs_w, const uint32_t* __restrict__ hdr, const int32_t* __restrict__ bperm,
@@ -187,7 +187,7 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
   const int dAB = kFull ? 128 : (actB ? chB : 0) - (actA ? chA : 0);
   const int sw = (int)lv.sw[level];
   const int sh = (int)lv.sh[level];
-  float* gtile = reinterpret_cast<float*>(const_cast<void*>(lv.data[level])) + (int64_t)n * lv.sn[level] +
+  G* gtile = reinterpret_cast<G*>(const_cast<void*>(lv.data[level])) + (int64_t)n * lv.sn[level] +
                  (int64_t)y0 * sh + (int64_t)x0 * sw + chA;
   const int npx = x1 - x0 + 1, npy = y1 - y0 + 1;
 
@@ -204,9 +204,9 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
       for (int i = 0; i < npy; ++i) {
         const int j = (warp + i) & 7;
         if (j >= npx) continue;
-        float* gp = gtile + i * sh + j * sw;
-        if (actA) *reinterpret_cast<float4*>(gp) = q4;
-        if (actB) *reinterpret_cast<float4*>(gp + 128) = q4;
+        G* gp = gtile + i * sh + j * sw;
+        if (actA) Grad4<G>::store(gp, q4);
+        if (actB) Grad4<G>::store(gp + 128, q4);
       }
       return;   // (uniform over the CTA: every warp sees the same words)
     }
@@ -324,11 +324,11 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
         const int j = (warp + i) & 7;
         if (j >= npx) continue;
         const int p = i * 8 + j;
-        float* gp = gtile + i * sh + j * sw;
+        G* gp = gtile + i * sh + j * sw;
         float4 accA = make_float4(0.f, 0.f, 0.f, 0.f), accB = accA;
         if (accumulate || npass) {
-          if (actA) accA = *reinterpret_cast<const float4*>(gp);
-          if (actB) accB = *reinterpret_cast<const float4*>(gp + 128);
+          if (actA) accA = Grad4<G>::load(gp);
+          if (actB) accB = Grad4<G>::load(gp + 128);
         }
         // pair count of every candidate on this pixel: lane c holds candidate c's
         const unsigned pcv = (lane < nc) ? s_pc[p][lane] : 0u;
@@ -401,8 +401,8 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
             }
           }
         }
-        if (actA) *reinterpret_cast<float4*>(gp) = accA;
-        if (actB) *reinterpret_cast<float4*>(gp + 128) = accB;
+        if (actA) Grad4<G>::store(gp, accA);
+        if (actB) Grad4<G>::store(gp + 128, accB);
       }
       ++npass;
       if (p0 + kNC < ncand || s0 + 2 * kPullThreads < bend)
@@ -415,9 +415,9 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
     for (int i = 0; i < npy; ++i) {
       const int j = (warp + i) & 7;
       if (j >= npx) continue;
-      float* gp = gtile + i * sh + j * sw;
-      if (actA) *reinterpret_cast<float4*>(gp) = z;
-      if (actB) *reinterpret_cast<float4*>(gp + 128) = z;
+      G* gp = gtile + i * sh + j * sw;
+      if (actA) Grad4<G>::store(gp, z);
+      if (actB) Grad4<G>::store(gp + 128, z);
     }
   }
 }
@@ -474,7 +474,7 @@ int pull_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a
   return pull_plan(glv, a, gout_strides, &pl);
 }
 
-template <typename T>
+template <typename T, typename G>
 static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout, const int64_t* gs,
                       const PullPrepOut& prep, int accumulate, cudaStream_t stream) {
   PullPlan pl;
@@ -483,9 +483,9 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
   const T* g = reinterpret_cast<const T*>(gout);
   const bool three = a.PH > 8 || a.PW > 8;
 #define RAF_LAUNCH_PULL(FULL, THREE)                                                                                      \
-  bwd_pull_kernel<T, FULL, THREE><<<pl.grid, kPullThreads, pl.smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], \
-                                                                               prep.hdr, prep.bperm, prep.boff, prep.bwin, \
-                                                                               prep.taps, pl.t, accumulate, prep.fp)
+  bwd_pull_kernel<T, G, FULL, THREE><<<pl.grid, kPullThreads, pl.smem, stream>>>(lv, a, g, (int)gs[0], (int)gs[2], (int)gs[3], \
+                                                                                  prep.hdr, prep.bperm, prep.boff, prep.bwin, \
+                                                                                  prep.taps, pl.t, accumulate, prep.fp)
   if (lv.c % 256 == 0) { if (three) RAF_LAUNCH_PULL(true, true); else RAF_LAUNCH_PULL(true, false); }
   else { if (three) RAF_LAUNCH_PULL(false, true); else RAF_LAUNCH_PULL(false, false); }
 #undef RAF_LAUNCH_PULL
@@ -493,12 +493,16 @@ static int pull_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout,
   return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;
 }
 
-int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
+// grad_dtype: RAF_F32, or the 16-bit type of grad_out (checked by the caller).
+int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, raf_dtype grad_dtype, const RoiArgs& a, const void* grad_out,
                          const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream) {
+  const bool g32 = grad_dtype == RAF_F32;
   switch (gout_dtype) {
-    case RAF_F32: return pull_typed<float>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
-    case RAF_F16: return pull_typed<__half>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
-    case RAF_BF16: return pull_typed<__nv_bfloat16>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
+    case RAF_F32: return pull_typed<float, float>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
+    case RAF_F16: return g32 ? pull_typed<__half, float>(glv, a, grad_out, gout_strides, prep, accumulate, stream)
+                             : pull_typed<__half, __half>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
+    case RAF_BF16: return g32 ? pull_typed<__nv_bfloat16, float>(glv, a, grad_out, gout_strides, prep, accumulate, stream)
+                              : pull_typed<__nv_bfloat16, __nv_bfloat16>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
   }
   return RAF_ERR_DTYPE;
 }

@@ -71,7 +71,7 @@ constexpr int kWorkCap = RAF_STRIP_WORK;       // work-list items per flush (>= 
 constexpr int kScanRounds = 9;                 // bucket records per lane and round trip
 
 struct StripLevels {
-  float* data[kMaxLevels];
+  void* data[kMaxLevels];
   int64_t sn[kMaxLevels];
   int32_t sh[kMaxLevels], sw[kMaxLevels];
   int32_t h[kMaxLevels], w[kMaxLevels];
@@ -161,7 +161,7 @@ __host__ __device__ inline size_t strip_warp_smem(int NC, int PH, int PW, size_t
 __device__ __forceinline__ int strip_pow2_lanes(int P) { return P <= 8 ? 8 : (P <= 16 ? 16 : 32); }
 
 
-template <typename T, bool kFull>
+template <typename T, typename G, bool kFull>
 __global__ void __launch_bounds__(32 * kStripWarps)
 bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const T* __restrict__ gout, int gs_k, int gs_h,
                  int gs_w, const uint32_t* __restrict__ hdr, const int32_t* __restrict__ bperm,
@@ -209,7 +209,7 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
   const bool actA = kFull || chA < sl.C, actB = kFull || chB < sl.C;
   const T* goutA = gout + (actA ? chA : 0);
   const int sw = sl.sw[level], sh = sl.sh[level];
-  float* gtile = sl.data[level] + (int64_t)n * sl.sn[level] + (int64_t)y0 * sh + (int64_t)x0 * sw + chA;
+  G* gtile = reinterpret_cast<G*>(sl.data[level]) + (int64_t)n * sl.sn[level] + (int64_t)y0 * sh + (int64_t)x0 * sw + chA;
 
   const int key = level * sl.N + n;
   const int bbeg = __ldg(boff + key), bend = __ldg(boff + key + 1);
@@ -230,17 +230,17 @@ bwd_strip_kernel(const __grid_constant__ StripLevels sl, const RoiArgs a, const 
     }
   };
   auto store_row = [&](int r, bool add_old) {
-    float* gp = gtile + r * sh;
+    G* gp = gtile + r * sh;
 #pragma unroll
     for (int j = 0; j < kStripCols; ++j) {
       if (j < npx) {
         float4 vA = acc[j][0], vB = acc[j][1];
         if (add_old) {
-          if (actA) { const float4 o = *reinterpret_cast<const float4*>(gp); vA.x += o.x; vA.y += o.y; vA.z += o.z; vA.w += o.w; }
-          if (actB) { const float4 o = *reinterpret_cast<const float4*>(gp + 128); vB.x += o.x; vB.y += o.y; vB.z += o.z; vB.w += o.w; }
+          if (actA) { const float4 o = Grad4<G>::load(gp); vA.x += o.x; vA.y += o.y; vA.z += o.z; vA.w += o.w; }
+          if (actB) { const float4 o = Grad4<G>::load(gp + 128); vB.x += o.x; vB.y += o.y; vB.z += o.z; vB.w += o.w; }
         }
-        if (actA) *reinterpret_cast<float4*>(gp) = vA;
-        if (actB) *reinterpret_cast<float4*>(gp + 128) = vB;
+        if (actA) Grad4<G>::store(gp, vA);
+        if (actB) Grad4<G>::store(gp + 128, vB);
       }
       gp += sw;
     }
@@ -477,7 +477,7 @@ static int strip_plan(const LevelsParam& lv, const RoiArgs& a, const int64_t* gs
   for (int i = 0; i < lv.L; ++i) {
     const int l = lv.L - 1 - i;  // coarsest level first
     t.order[i] = l;
-    t.data[l] = reinterpret_cast<float*>(const_cast<void*>(lv.data[l]));
+    t.data[l] = const_cast<void*>(lv.data[l]);
     t.sn[l] = lv.sn[l];
     if (lv.sh[l] >= ((int64_t)1 << 31) || lv.sw[l] >= ((int64_t)1 << 31)) return RAF_ERR_UNSUPPORTED;
     t.sh[l] = (int32_t)lv.sh[l]; t.sw[l] = (int32_t)lv.sw[l];
@@ -517,7 +517,7 @@ int strip_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& 
   return strip_plan(glv, a, gout_strides, gout_dtype == RAF_F32 ? 4 : 2, &pl);
 }
 
-template <typename T>
+template <typename T, typename G>
 static int strip_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout, const int64_t* gs,
                        const PullPrepOut& prep, int accumulate, cudaStream_t stream) {
   StripPlan pl;
@@ -527,10 +527,10 @@ static int strip_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout
 #define RAF_LAUNCH_STRIP(FULL)                                                                                   \
   do {                                                                                                           \
     if (pl.smem > 48 * 1024 &&                                                                                   \
-        cudaFuncSetAttribute(bwd_strip_kernel<T, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize,             \
+        cudaFuncSetAttribute(bwd_strip_kernel<T, G, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
                              (int)pl.smem) != cudaSuccess)                                                       \
       return RAF_ERR_CUDA;                                                                                       \
-    bwd_strip_kernel<T, FULL><<<pl.grid, 32 * kStripWarps, pl.smem, stream>>>(                                   \
+    bwd_strip_kernel<T, G, FULL><<<pl.grid, 32 * kStripWarps, pl.smem, stream>>>(                                \
         pl.sl, a, g, (int)gs[0], (int)gs[2], (int)gs[3], prep.hdr, prep.bperm, prep.boff, prep.bwin, prep.bgeo,  \
         pl.NC, accumulate, prep.fp);                                                                             \
   } while (0)
@@ -541,12 +541,16 @@ static int strip_typed(const LevelsParam& lv, const RoiArgs& a, const void* gout
   return cudaGetLastError() == cudaSuccess ? RAF_OK : RAF_ERR_CUDA;
 }
 
-int launch_backward_strip(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
+// grad_dtype: RAF_F32, or the 16-bit type of grad_out (checked by the caller).
+int launch_backward_strip(const LevelsParam& glv, raf_dtype gout_dtype, raf_dtype grad_dtype, const RoiArgs& a, const void* grad_out,
                           const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream) {
+  const bool g32 = grad_dtype == RAF_F32;
   switch (gout_dtype) {
-    case RAF_F32: return strip_typed<float>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
-    case RAF_F16: return strip_typed<__half>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
-    case RAF_BF16: return strip_typed<__nv_bfloat16>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
+    case RAF_F32: return strip_typed<float, float>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
+    case RAF_F16: return g32 ? strip_typed<__half, float>(glv, a, grad_out, gout_strides, prep, accumulate, stream)
+                             : strip_typed<__half, __half>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
+    case RAF_BF16: return g32 ? strip_typed<__nv_bfloat16, float>(glv, a, grad_out, gout_strides, prep, accumulate, stream)
+                              : strip_typed<__nv_bfloat16, __nv_bfloat16>(glv, a, grad_out, gout_strides, prep, accumulate, stream);
   }
   return RAF_ERR_DTYPE;
 }

@@ -188,6 +188,41 @@ template <> struct Vec16<__nv_bfloat16> {
   }
 };
 
+// 4 consecutive gradient channels of type G (the gradient pyramid is fp32, or -- roi_align_fpn_backward_ex -- the
+// 16-bit type of grad_out: sums are formed in fp32 registers and rounded once when they are stored).
+template <typename G> struct Grad4;
+template <> struct Grad4<float> {
+  static __device__ __forceinline__ float4 load(const float* p) { return *reinterpret_cast<const float4*>(p); }
+  static __device__ __forceinline__ void store(float* p, const float4& v) { *reinterpret_cast<float4*>(p) = v; }
+};
+template <> struct Grad4<__half> {
+  static __device__ __forceinline__ float4 load(const __half* p) {
+    const uint2 r = *reinterpret_cast<const uint2*>(p);
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+  }
+  static __device__ __forceinline__ void store(__half* p, const float4& v) {
+    uint2 r;
+    *reinterpret_cast<__half2*>(&r.x) = __floats2half2_rn(v.x, v.y);
+    *reinterpret_cast<__half2*>(&r.y) = __floats2half2_rn(v.z, v.w);
+    *reinterpret_cast<uint2*>(p) = r;
+  }
+};
+template <> struct Grad4<__nv_bfloat16> {
+  static __device__ __forceinline__ float4 load(const __nv_bfloat16* p) {
+    const uint2 r = *reinterpret_cast<const uint2*>(p);
+    return make_float4(__uint_as_float(r.x << 16), __uint_as_float(r.x & 0xffff0000u),
+                       __uint_as_float(r.y << 16), __uint_as_float(r.y & 0xffff0000u));
+  }
+  static __device__ __forceinline__ void store(__nv_bfloat16* p, const float4& v) {
+    uint2 r;
+    *reinterpret_cast<__nv_bfloat162*>(&r.x) = __floats2bfloat162_rn(v.x, v.y);
+    *reinterpret_cast<__nv_bfloat162*>(&r.y) = __floats2bfloat162_rn(v.z, v.w);
+    *reinterpret_cast<uint2*>(p) = r;
+  }
+};
+
 // fp32 vector reduction into global memory (sm_90+): one L2 atomic transaction for 16 bytes.
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c),

@@ -57,13 +57,13 @@ int pull_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a
 // gradient element exactly once (or adds into it when `accumulate`).  `prep` = the tables
 // launch_pull_prep (or the forward) left in the workspace for the same arguments, with the
 // fingerprint the kernel checks them against.
-int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
+int launch_backward_pull(const LevelsParam& glv, raf_dtype gout_dtype, raf_dtype grad_dtype, const RoiArgs& a, const void* grad_out,
                          const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream);
 
 // Second-generation pull backward (raf_backward_strip.cu): row-strip register accumulators, each grad_out
 // vector loaded once per strip.  Same prep tables (bperm / boff / bwin / bgeo), same fingerprint check.
 int strip_eligible(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const int64_t* gout_strides);
-int launch_backward_strip(const LevelsParam& glv, raf_dtype gout_dtype, const RoiArgs& a, const void* grad_out,
+int launch_backward_strip(const LevelsParam& glv, raf_dtype gout_dtype, raf_dtype grad_dtype, const RoiArgs& a, const void* grad_out,
                           const int64_t* gout_strides, const PullPrepOut& prep, int accumulate, cudaStream_t stream);
 
 // RoIPool-max (raf_pool.cu).  `chan_fastest`: enumerate outputs with the channel fastest (channels-last

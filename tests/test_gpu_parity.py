@@ -659,3 +659,57 @@ def test_repack_nchw_forward_and_backward(dtype):
     gref, S = R.backward(cfg.level_shapes, cfg.scales, go_t.to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
                          cfg.finest_scale)
     T.assert_backward_close([t.to(torch.float64).cpu().numpy() for t in g_nchw], gref, S)
+
+
+@pytest.mark.parametrize("variant", [B.RAF_PULL_TILE, B.RAF_PULL_STRIP])
+@pytest.mark.parametrize("index,dtype,kw,P", [
+    (4, "bf16", dict(n_img=2, per_img=40, channels=32), None),
+    (5, "bf16", dict(n_img=3, per_img=64, channels=64), None),
+    (5, "f16", dict(n_img=2, per_img=50, channels=36), None),
+    (5, "bf16", dict(n_img=1, per_img=400, channels=16), (7, 7)),     # dense: tiles with several passes / batches
+])
+def test_backward_16bit_gradient_pyramid(index, dtype, kw, P, variant):
+    """roi_align_fpn_backward_ex with the gradient pyramid in grad_out's 16-bit type: fp32 sums
+    rounded once per element and pass.  Tolerance: 16-bit rounding of the result (2e-2 relative, north_star's
+    figure for 16-bit outputs) + one rounding of a partial sum per extra pass (eps_16 * S, S = sum |terms|)."""
+    wl = inputs.make_workload(index, **kw)
+    cfg = wl.cfg
+    tdt = T.TORCH_DTYPE[dtype]
+    PH, PW = P or cfg.out_size
+    K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
+    rng = np.random.default_rng(17)
+    gout_np = wl.grad_out if (PH, PW) == tuple(cfg.out_size) else rng.standard_normal((K, C, PH, PW)).astype(np.float32)
+    rois = torch.from_numpy(wl.rois).cuda()
+    go_t = torch.from_numpy(gout_np).to(tdt)
+    go = T.to_layout(go_t.cuda(), "cl")
+    ws = T.workspace(K, L, PH, PW, 2)
+    gref, S = R.backward(cfg.level_shapes, cfg.scales, go_t.to(torch.float64).numpy(), wl.rois, (PH, PW), 2, True,
+                         cfg.finest_scale)
+    eps = 2.0 ** -8 if dtype == "bf16" else 2.0 ** -11
+    for accumulate in (False, True):
+        init = [rng.standard_normal(s).astype(np.float32) for s in cfg.level_shapes]
+        if accumulate:
+            grads = [T.to_layout(torch.from_numpy(x).to(tdt).cuda(), "cl") for x in init]
+            start = [g.to(torch.float64).cpu().numpy() for g in grads]
+        else:
+            grads = [T.empty_layout(s, tdt, "cl", fill=float("nan")) for s in cfg.level_shapes]
+            start = [np.zeros(s) for s in cfg.level_shapes]
+        B.roi_align_fpn_backward(grads, cfg.scales, go, rois, 2, True, cfg.finest_scale,
+                                 variant | (B.RAF_ACCUMULATE if accumulate else 0), ws)
+        torch.cuda.synchronize()
+        for g, r, s, st in zip(grads, gref, S, start):
+            got = g.to(torch.float64).cpu().numpy()
+            want = r + st
+            assert np.isfinite(got).all()
+            tol = 2e-2 * np.abs(want) + 4 * eps * (s + np.abs(st)) + 1e-6
+            assert (np.abs(got - want) <= tol).all(), float((np.abs(got - want) / tol).max())
+            if not accumulate:
+                assert np.all(got[s == 0] == 0)
+    # the combinations the header rules out
+    g32 = [T.empty_layout(s, torch.float32, "cl") for s in cfg.level_shapes]
+    with pytest.raises(B.RafError) as e:
+        B.roi_align_fpn_backward([T.empty_layout(s, tdt, "cl") for s in cfg.level_shapes], cfg.scales, go, rois, 2, True,
+                                 cfg.finest_scale, B.RAF_ATOMIC, ws)
+    assert e.value.status == -5
+    with pytest.raises(ValueError):
+        B.roi_align_fpn_backward([t.to(torch.float64) for t in g32], cfg.scales, go, rois, 2, True, cfg.finest_scale, 0, ws)

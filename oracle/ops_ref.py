@@ -129,3 +129,34 @@ def deform_roi_pool_backward(feats, scales, grad_out, rois, offset, gamma, sampl
                                                 int(sampling_ratio), ctypes.c_float(finest_scale), int(bool(f64)), _p(goff))
     assert rc == 0
     return grads, goff
+
+
+def _round_to(x64, dtype):
+    """float64 -> the value a 16-bit (or fp32) store keeps, returned as float64 (round to nearest even)."""
+    if dtype == "f32":
+        return x64.astype(np.float32).astype(np.float64)
+    if dtype == "f16":
+        return x64.astype(np.float16).astype(np.float64)
+    assert dtype == "bf16"
+    u = x64.astype(np.float32).view(np.uint32).astype(np.uint64)
+    u = ((u + 0x7FFF + ((u >> 16) & 1)) >> 16) << 16          # round to nearest even on the upper 16 bits
+    return u.astype(np.uint32).view(np.float32).astype(np.float64)
+
+
+def roi_align_fc_forward(feats, scales, rois, weight, bias, out_size, sampling_ratio, aligned, finest_scale=56.0,
+                         dtype="bf16"):
+    """RoIExtractor -> first FC of the box head (readings F1-F3), as a composition:
+    (1) RoIAlign forward of the pinned oracle (oracle/raf_ref.cpp, spec mode); (2) every feature rounded to `dtype`, as
+    the RoI feature tensor the head would read (F2); (3) flattened per RoI in (ph, pw, c) order (F1); (4) a library
+    matrix product in float64 with the weight [N_out, PH*PW*C] (+ bias).  Returns float64 [K, N_out]."""
+    from . import raf_ref as _raf
+    x = _raf.forward(feats, scales, rois, out_size, sampling_ratio, aligned, finest_scale, coord_f32=True)   # [K,C,PH,PW]
+    x = _round_to(x, dtype)
+    K = x.shape[0]
+    a = np.ascontiguousarray(x.transpose(0, 2, 3, 1)).reshape(K, -1)                                            # (ph, pw, c)
+    w = np.ascontiguousarray(weight, dtype=np.float64)
+    assert w.shape[1] == a.shape[1]
+    out = a @ w.T
+    if bias is not None:
+        out = out + np.asarray(bias, dtype=np.float64)[None, :]
+    return out

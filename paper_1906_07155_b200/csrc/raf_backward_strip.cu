@@ -40,7 +40,7 @@
 // Any sampling grid (fixed g >= 1, or the adaptive per-RoI grid of sampling_ratio == 0) and any
 // out_h / out_w <= 32 take this path (no tap-count limit).
 //
-// Measured (B200, cold-L2 rotation, profiles/r2_backward.md): config 5 (16 images, 25.8 K warp tiles)
+// Measured (B200, cold-L2 rotation, profiles/r2_experiments.md): config 5 (16 images, 25.8 K warp tiles)
 // 516 -> 455 us against the first generation; on config 2 (2 images, 3.2 K warp tiles = 1.8 waves of
 // 12 resident warps per SM) the fixed ~8 us of dependent round trips per tile is not covered and the
 // first generation stays ahead (89 vs 95 us), as it does for outputs finer than the pixel grid

@@ -386,3 +386,45 @@ def test_deform_backward_adjoint_and_finite_differences():
     # spec mode (fp32 coordinates) stays within coordinate rounding of the f64 mode
     gf32, goff32 = O.deform_roi_pool_backward(feats, scales, gout, rois, off, gamma, 2, f64=False)
     assert max(np.abs(a - b).max() for a, b in zip(gf, gf32)) < 1e-3
+
+
+# --------------------------------------------------------------------------- RoIAlign -> first FC (fused op)
+def test_roi_align_fc_oracle_flatten_order_rounding_and_linearity():
+    """Pins of O.roi_align_fc_forward (readings F1-F3): a selection matrix returns single rounded RoI features in
+    (ph, pw, c) order; the product is linear in the weight and adds the bias; a loop restatement on a tiny case."""
+    rng = np.random.default_rng(9)
+    feats = [rng.standard_normal((1, 8, 24, 30)), rng.standard_normal((1, 8, 12, 15))]
+    scales = [0.25, 0.125]
+    rois = np.array([[0, 10, 12, 70, 60], [0, 5, 5, 110, 90], [0, 30, 20, 50, 44]], np.float32)
+    P = (3, 4)
+    x = R.forward(feats, scales, rois, P, 2, True, 56.0, coord_f32=True)
+    Kd = P[0] * P[1] * 8
+    # selection: output n picks flattened index sel[n]
+    sel = np.array([0, 7, 8, 8 * 4 + 3, Kd - 1])
+    W = np.zeros((len(sel), Kd)); W[np.arange(len(sel)), sel] = 1.0
+    got = O.roi_align_fc_forward(feats, scales, rois, W, None, P, 2, True, dtype="bf16")
+    for n, s in enumerate(sel):
+        ph, pw, c = s // (P[1] * 8), (s // 8) % P[1], s % 8
+        want = x[:, c, ph, pw]
+        # bf16 keeps an 8-bit significand, round to nearest even (np.round rounds halves to even); the value is first
+        # rounded to fp32, which cannot move an 8-bit rounding decision except at exact ties (none in random data)
+        m, e = np.frexp(want)
+        q = np.ldexp(np.round(m * 256.0) / 256.0, e)
+        assert np.array_equal(got[:, n], q)
+    # f32 "rounding" keeps the features; linearity and bias
+    W1, W2 = rng.standard_normal((6, Kd)), rng.standard_normal((6, Kd))
+    b = rng.standard_normal(6)
+    f = lambda w, bb: O.roi_align_fc_forward(feats, scales, rois, w, bb, P, 2, True, dtype="f32")
+    assert np.abs(f(2 * W1 - W2, b) - (2 * f(W1, None) - f(W2, None) + b)).max() < 1e-9
+    # loop restatement
+    xr = x.astype(np.float32).astype(np.float64)
+    want = np.zeros((3, 6))
+    for k in range(3):
+        for n in range(6):
+            acc = 0.0
+            for ph in range(P[0]):
+                for pw in range(P[1]):
+                    for c in range(8):
+                        acc += xr[k, c, ph, pw] * W1[n, (ph * P[1] + pw) * 8 + c]
+            want[k, n] = acc
+    assert np.abs(f(W1, None) - want).max() < 1e-10

@@ -50,7 +50,7 @@ def parse_args():
     ap.add_argument("--rotate", type=int, default=0,
                     help="number of independent input/output buffer sets to rotate over (0 = cold-L2 protocol: "
                          "at least 4 and >= 2x L2; 1 = WARM single-buffer number, not the headline)")
-    ap.add_argument("--op", default="align", choices=["align", "pool", "deform", "nms", "softnms"],
+    ap.add_argument("--op", default="align", choices=["align", "pool", "deform", "fc", "nms", "softnms"],
                     help="align: the headline FPN RoIAlign fwd+bwd (BASELINE.json metric); pool / nms / softnms: the SURVEY 8(f) "
                          "operations, one extra bench line each (not the headline)")
     ap.add_argument("--nms-n", type=int, default=2000, help="boxes for --op nms / softnms")
@@ -577,6 +577,51 @@ def run_op(args):
                                      "windows differ by at most a pixel per side) + out + argmax written + grad_out + argmax "
                                      "read + gradient pyramid zero-filled and written"},
                 "clocks": clocks, "gpu_launches": args.windows * args.window_iters * (2 + len(cfg.level_shapes))}
+    elif args.op == "fc":
+        # RoIAlign gather fused into the box head's first FC (12544 -> 1024 for the 7 x 7 x 256 box head), bf16 features and
+        # weights, fp32 accumulate.  Context number in the same line: the library's stand-alone forward + a cuBLAS product.
+        cfg = inputs.CONFIGS[args.config]
+        wl = inputs.make_workload(args.config)
+        tdt = torch.bfloat16 if cfg.dtype == "f32" else {"f16": torch.float16, "bf16": torch.bfloat16}[cfg.dtype]
+        K, C = cfg.K, cfg.channels
+        PH, PW = cfg.out_size
+        n_out = 1024
+        lay = lambda t: t.permute(0, 2, 3, 1).contiguous().permute(0, 3, 1, 2)
+        R = 4
+        feats = [[lay(torch.from_numpy(f).to(tdt).cuda()) for f in wl.feats] for _ in range(R)]
+        rois = torch.from_numpy(wl.rois).cuda()
+        rng = np.random.default_rng(190607155 + 79)
+        w = torch.from_numpy((rng.standard_normal((n_out, PH * PW * C)) / np.sqrt(PH * PW * C)).astype(np.float32)).to(tdt).cuda()
+        bias = torch.from_numpy(rng.standard_normal(n_out).astype(np.float32)).cuda()
+        outs = [torch.empty((K, n_out), dtype=torch.float32, device="cuda") for _ in range(R)]
+        xs = [lay(torch.empty((K, C, PH, PW), dtype=tdt, device="cuda")) for _ in range(R)]
+
+        def step(j):
+            B.roi_align_fc_fpn_forward(feats[j], cfg.scales, rois, w, bias, outs[j], (PH, PW), 2, True, cfg.finest_scale, stream)
+
+        def unfused(j):
+            B.roi_align_fpn_forward_ex(feats[j], cfg.scales, rois, xs[j], 2, True, cfg.finest_scale, B.RAF_NO_PREP, None, stream)
+            torch.addmm(bias.to(tdt), xs[j].permute(0, 2, 3, 1).reshape(K, -1), w.t())
+        ms, ms_min, clocks = timed(step, R)
+        ms_unf, _, _ = timed(unfused, R)
+        flops = 2.0 * K * PH * PW * C * n_out
+        tensor_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("bf16_tflops") if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else None
+        tpeak = float(tensor_peak) if tensor_peak else 2250.0
+        line = {"metric": "RoIAlign + first FC (12544 -> 1024) RoIs/sec, fused gather + tcgen05 GEMM", "value": K / (ms * 1e-3),
+                "unit": UNIT, "n_gpus": 1, "steps": args.windows * args.window_iters, "warmup": max(args.warmup, 3),
+                "ms_per_step": ms, "ms_per_step_min": ms_min, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "bf16" if tdt == torch.bfloat16 else "f16", "data": "synthetic",
+                "config": {"workload": f"fused RoIAlign + FC on BASELINE.json configs[{args.config - 1}] shapes (features cast to 16 bit): {cfg.name}",
+                           "K": K, "C": C, "out_size": [PH, PW], "n_out": n_out, "layout": "cl",
+                           "l2_protocol": f"inputs rotate over {R} independent copies",
+                           "unfused_context_ms": ms_unf,
+                           "unfused_context": "roi_align_fpn_forward_ex(RAF_NO_PREP) + torch.addmm (cuBLAS), same inputs"},
+                "roofline": {"bound": "tensor", "kernel": "fc_fused_kernel", "achieved": flops / (ms * 1e-3) / 1e12, "peak": tpeak,
+                             "unit": "TFLOP/s", "frac": flops / (ms * 1e-3) / 1e12 / tpeak, "traffic": None,
+                             "note": "flops of the matrix product only; the kernel is bound by its gathers (every RoI window "
+                                     "is gathered n_out / 256 times), not by the tensor cores",
+                             "peak_source": "MEASURED_PEAKS.json bf16_tflops" if tensor_peak else "nominal 2250 TFLOP/s dense bf16"},
+                "clocks": clocks, "gpu_launches": args.windows * args.window_iters * 2}
     elif args.op == "deform":
         cfg = inputs.CONFIGS[args.config]
         wl = inputs.make_workload(args.config)

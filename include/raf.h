@@ -176,6 +176,22 @@ int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dty
                           const int32_t* argmax, const int64_t* gout_strides, const float* rois, int K,
                           int out_h, int out_w, float finest_scale, int flags, void* stream);
 
+/* ---- the RoIAlign gather fused into the box head's first fully connected layer (RoIHead /
+ * BBoxHead; "2fc" heads PAPER.md:269-271).  Readings F1-F3:
+ *   out[k, n] = sum_{ph,pw,c} A[k, (ph*out_w + pw)*C + c] * weight[n, (ph*out_w + pw)*C + c]  (+ bias[n])
+ * with A = the RoIAlign forward of RoI k (same definition as roi_align_fpn_forward) ROUNDED to `dtype`, i.e. exactly
+ * the RoI feature tensor the head would read -- but it is never written: tiles of it are produced straight into the
+ * A operand of a tcgen05 GEMM (bf16 / fp16 inputs, fp32 accumulation in tensor memory).
+ *   feats    channels-last (sc == 1), dtype RAF_F16 or RAF_BF16, C % 64 == 0
+ *   weight   DEVICE, dtype, [n_out, out_h*out_w*C] row-major, columns in (ph, pw, c) order; n_out % 256 == 0
+ *   bias     DEVICE fp32 [n_out] or NULL
+ *   out      DEVICE fp32 [K, n_out] row-major, overwritten (zero-filled, then fp32 reductions: the summation order
+ *            over the out_h split-K slices is not fixed)
+ *   sampling_ratio 1 or 2.  Anything else: RAF_ERR_UNSUPPORTED. */
+int roi_align_fc_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                             int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
+                             const void* weight, const float* bias, int n_out, float* out, void* stream);
+
 /* ---- deformable RoI pooling ("DCN [8]: deformable convolution and deformable RoI pooling",
  * PAPER.md:57-58), on the same FPN level map (C1).  Readings D1-D5: RoIAlign with the half-pixel
  * shift and no minimum size whose bin (ph,pw) is moved by (gamma*rw*offset[k,0,ph,pw], gamma*rh*offset[k,1,ph,pw])

@@ -26,6 +26,7 @@ EXPORTS = [
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
     "roi_pool_fpn_forward", "roi_pool_fpn_backward", "roi_nms_workspace_bytes", "roi_nms", "roi_soft_nms",
     "roi_align_fpn_repack_bytes", "roi_deform_pool_fpn_forward", "roi_deform_pool_fpn_backward",
+    "roi_align_fc_fpn_forward",
 ]
 
 
@@ -87,6 +88,8 @@ def lib() -> ctypes.CDLL:
         L.roi_deform_pool_fpn_forward.argtypes = [vp, ci, ci, vp, ci, vp, cf, ci, ci, ci, cf, vp, vp, vp]
         L.roi_deform_pool_fpn_backward.restype = ci
         L.roi_deform_pool_fpn_backward.argtypes = [vp, vp, ci, ci, vp, vp, vp, ci, vp, cf, ci, ci, ci, cf, vp, ci, vp]
+        L.roi_align_fc_fpn_forward.restype = ci
+        L.roi_align_fc_fpn_forward.argtypes = [vp, ci, ci, vp, ci, ci, ci, ci, ci, cf, vp, vp, ci, vp, vp]
         L.roi_nms_workspace_bytes.restype = ctypes.c_size_t
         L.roi_nms_workspace_bytes.argtypes = [ci]
         L.roi_nms.restype = ci
@@ -362,6 +365,34 @@ def roi_deform_pool_fpn_backward(feats: Sequence[torch.Tensor], grad_feats: Opti
                                             _ptr(grad_offset), int(flags), _stream_ptr(stream))
     if rc:
         raise RafError(rc, "roi_deform_pool_fpn_backward")
+
+
+def roi_align_fc_fpn_forward(feats: Sequence[torch.Tensor], scales: Sequence[float], rois: torch.Tensor,
+                             weight: torch.Tensor, bias: Optional[torch.Tensor], out: torch.Tensor, out_size,
+                             sampling_ratio: int, aligned: bool, finest_scale: float, stream=None) -> None:
+    """RoIAlign gather fused into the first FC (include/raf.h).  weight: [n_out, PH*PW*C] in the feature dtype, columns in
+    (ph, pw, c) order; bias: float32 [n_out] or None; out: float32 [K, n_out] contiguous."""
+    if len(feats) == 0 or feats[0].dtype not in _DTYPES:
+        raise ValueError("unsupported feature dtype")
+    PH, PW = out_size
+    K, C = rois.shape[0], feats[0].shape[1]
+    if rois.dtype != torch.float32 or rois.dim() != 2 or rois.shape[1] != 5 or not rois.is_contiguous():
+        raise ValueError("rois must be a contiguous float32 [K,5] tensor")
+    if (weight.dtype != feats[0].dtype or weight.dim() != 2 or weight.shape[1] != PH * PW * C or not weight.is_contiguous()):
+        raise ValueError("weight must be a contiguous [n_out, PH*PW*C] tensor of the feature dtype")
+    n_out = weight.shape[0]
+    if bias is not None and (bias.dtype != torch.float32 or tuple(bias.shape) != (n_out,) or not bias.is_contiguous()):
+        raise ValueError("bias must be a contiguous float32 [n_out] tensor")
+    if out.dtype != torch.float32 or tuple(out.shape) != (K, n_out) or not out.is_contiguous():
+        raise ValueError("out must be a contiguous float32 [K, n_out] tensor")
+    tensors = list(feats) + [rois, weight, out] + ([bias] if bias is not None else [])
+    if not all(t.is_cuda for t in tensors) or len({t.device for t in tensors}) != 1:
+        raise ValueError("all tensors must live on the same CUDA device")
+    rc = lib().roi_align_fc_fpn_forward(make_levels(feats, scales), len(feats), _DTYPES[feats[0].dtype], _ptr(rois), K, PH, PW,
+                                        int(sampling_ratio), int(bool(aligned)), finest_scale, _ptr(weight), _ptr(bias),
+                                        n_out, _ptr(out), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fc_fpn_forward")
 
 
 def _check_boxes(boxes: torch.Tensor, scores: torch.Tensor) -> int:

@@ -474,6 +474,30 @@ int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dty
                               unit_channel_stride(grad_feats, L), st);
 }
 
+// ---- RoIAlign gather fused into the first FC ------------------------------------------------------------
+int roi_align_fc_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
+                             int out_h, int out_w, int sampling_ratio, int aligned, float finest_scale,
+                             const void* weight, const float* bias, int n_out, float* out, void* stream) {
+  int rc = check_levels(feats, L);
+  if (rc) return rc;
+  rc = check_common(rois, K, out_h, out_w, sampling_ratio);
+  if (rc) return rc;
+  if (dtype != RAF_F32 && dtype != RAF_F16 && dtype != RAF_BF16) return RAF_ERR_DTYPE;
+  if (!(finest_scale > 0.0f) || n_out < 1) return RAF_ERR_SHAPE;
+  if (K == 0) return RAF_OK;
+  if (!weight || !out) return RAF_ERR_NULL;
+  if (dtype == RAF_F32 || sampling_ratio < 1 || sampling_ratio > 2 || n_out % 256 || feats[0].c % 64) return RAF_ERR_UNSUPPORTED;
+  if (!levels_vectorizable(feats, L, 8, 2) || ((uintptr_t)weight) % 16 || ((uintptr_t)out) % 16) return RAF_ERR_UNSUPPORTED;
+  if ((int64_t)K * n_out >= ((int64_t)1 << 40)) return RAF_ERR_UNSUPPORTED;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (cudaMemsetAsync(out, 0, sizeof(float) * (size_t)K * n_out, st) != cudaSuccess) return RAF_ERR_CUDA;
+  count_launch();
+  LevelsParam p;
+  fill_param(feats, L, &p);
+  const RoiArgs a{rois, K, out_h, out_w, sampling_ratio, aligned ? 1 : 0, finest_scale};
+  return launch_fc_fused(p, dtype, a, weight, bias, n_out, out, st);
+}
+
 // ---- deformable RoI pooling ---------------------------------------------------------------------------
 int roi_deform_pool_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, const float* rois, int K,
                                 const float* offset, float gamma, int out_h, int out_w, int sampling_ratio,

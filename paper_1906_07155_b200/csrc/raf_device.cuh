@@ -160,6 +160,12 @@ template <> struct Vec16<__half> {
 #pragma unroll
     for (int i = 0; i < 4; ++i) { const float2 f = __half22float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
   }
+  static __device__ __forceinline__ uint4 load_raw(const __half* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+  static __device__ __forceinline__ void widen(const uint4& r, float (&v)[8]) {
+    const __half2* h = reinterpret_cast<const __half2*>(&r);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { const float2 f = __half22float2(h[i]); v[2 * i] = f.x; v[2 * i + 1] = f.y; }
+  }
   static __device__ __forceinline__ void store(__half* p, const float (&v)[8]) {
     uint4 r;
     __half2* h = reinterpret_cast<__half2*>(&r);
@@ -175,6 +181,15 @@ template <> struct Vec16<__nv_bfloat16> {
     const uint32_t* u = reinterpret_cast<const uint32_t*>(&r);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {  // bf16 -> fp32 is a 16-bit shift
+      v[2 * i] = __uint_as_float(u[i] << 16);
+      v[2 * i + 1] = __uint_as_float(u[i] & 0xffff0000u);
+    }
+  }
+  static __device__ __forceinline__ uint4 load_raw(const __nv_bfloat16* p) { return __ldg(reinterpret_cast<const uint4*>(p)); }
+  static __device__ __forceinline__ void widen(const uint4& r, float (&v)[8]) {
+    const uint32_t* u = reinterpret_cast<const uint32_t*>(&r);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
       v[2 * i] = __uint_as_float(u[i] << 16);
       v[2 * i + 1] = __uint_as_float(u[i] & 0xffff0000u);
     }

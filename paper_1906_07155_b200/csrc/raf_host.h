@@ -80,6 +80,10 @@ int launch_deform_backward(const LevelsParam& lv, const LevelsParam& glv, bool w
                            int K, const float* offset, float gamma, int PH, int PW, int g, float fs, const void* gout,
                            const int64_t* gs, float* grad_offset, bool chan_fastest, cudaStream_t stream);
 
+// RoIAlign gather fused into the box head's first FC (raf_fc.cu; tcgen05).  `out` must already be zero.
+int launch_fc_fused(const LevelsParam& lv, raf_dtype dtype, const RoiArgs& a, const void* W, const float* bias, int n_out,
+                    float* out, cudaStream_t stream);
+
 // NMS / Soft-NMS (raf_nms.cu).
 size_t nms_workspace_bytes(int n);
 int launch_nms(const float* boxes, const float* scores, int n, float iou_threshold, int32_t* keep, int32_t* num_keep,

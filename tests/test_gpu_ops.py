@@ -236,3 +236,86 @@ def test_deform_roi_pool_argument_errors():
     with pytest.raises(B.RafError) as e:
         B.roi_deform_pool_fpn_backward(feats, None, cfg.scales, go, rois, None, 0.1, 2, 56.0, None, flags=B.RAF_ATOMIC)
     assert e.value.status == -5
+
+
+# ----------------------------------------------------------------- RoIAlign gather fused into the first FC
+def _fc_case(index, dtype, kw, n_out, g=2, bias=True, seed=0):
+    wl = inputs.make_workload(index, **kw)
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C = cfg.K, cfg.channels
+    tdt = T.TORCH_DTYPE[dtype]
+    rng = np.random.default_rng(seed)
+    feats, exact = T.device_feats(wl.feats, dtype, "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    w_t = torch.from_numpy((rng.standard_normal((n_out, PH * PW * C)) / np.sqrt(PH * PW * C)).astype(np.float32)).to(tdt)
+    b_np = rng.standard_normal(n_out).astype(np.float32) if bias else None
+    out = torch.full((K, n_out), float("nan"), dtype=torch.float32, device="cuda")
+    B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w_t.cuda(), None if b_np is None else torch.from_numpy(b_np).cuda(), out,
+                               (PH, PW), g, True, cfg.finest_scale)
+    torch.cuda.synchronize()
+    w64 = w_t.to(torch.float64).numpy()
+    ref = O.roi_align_fc_forward(exact, cfg.scales, wl.rois, w64, b_np, (PH, PW), g, True, cfg.finest_scale, dtype=dtype)
+    # scale of the sum: sum |a| |w| with |a| <= the rounded features
+    refabs = O.roi_align_fc_forward([np.abs(e) for e in exact], cfg.scales, wl.rois, np.abs(w64), None if b_np is None else np.abs(b_np),
+                                    (PH, PW), g, True, cfg.finest_scale, dtype=dtype)
+    got = out.to(torch.float64).cpu().numpy()
+    assert np.isfinite(got).all()
+    # fp32 accumulation of PH*PW*C terms + a 16-bit rounding of a feature that sits next to a rounding boundary
+    # (the CUDA forward and the oracle agree to 1e-5 relative BEFORE rounding): |err| <= 2e-2 |ref| + 2e-3 * sum |terms|
+    eps = 2.0 ** -8 if dtype == "bf16" else 2.0 ** -11
+    tol = 2e-2 * np.abs(ref) + eps * refabs + 1e-5
+    err = np.abs(got - ref)
+    assert (err <= tol).all(), float((err / tol).max())
+    return float((err / tol).max()), float(err.max()), float(np.abs(ref).max())
+
+
+@pytest.mark.parametrize("index,dtype,kw,n_out,g", [
+    (5, "bf16", dict(n_img=2, per_img=100, channels=64), 256, 2),      # 200 RoIs: two M tiles, the second ragged
+    (4, "bf16", dict(n_img=1, per_img=40, channels=128), 512, 2),      # 14 x 14 bins, two N tiles
+    (3, "f16", dict(n_img=1, per_img=130, channels=64), 256, 2),
+    (5, "f16", dict(n_img=2, per_img=30, channels=192), 256, 1),
+])
+def test_roi_align_fc_fused(index, dtype, kw, n_out, g):
+    worst, emax, rmax = _fc_case(index, dtype, kw, n_out, g)
+    assert emax <= 2e-2 * rmax
+
+
+def test_roi_align_fc_fused_matches_unfused_library_path():
+    """The same numbers from the library's own RoIAlign forward followed by a matrix product (torch, fp32 accumulate):
+    the fused A tiles are bit-identical to the stand-alone forward's output, so the two differ only by the order of the
+    fp32 sums."""
+    wl = inputs.make_workload(5, n_img=2, per_img=64, channels=64)
+    cfg = wl.cfg
+    PH, PW = cfg.out_size
+    K, C = cfg.K, cfg.channels
+    feats, _ = T.device_feats(wl.feats, "bf16", "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    rng = np.random.default_rng(3)
+    w = torch.from_numpy((rng.standard_normal((256, PH * PW * C)) / 56.0).astype(np.float32)).to(torch.bfloat16).cuda()
+    out = torch.empty((K, 256), dtype=torch.float32, device="cuda")
+    B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w, None, out, (PH, PW), 2, True, cfg.finest_scale)
+    x = T.empty_layout((K, C, PH, PW), torch.bfloat16, "cl")
+    B.roi_align_fpn_forward_ex(feats, cfg.scales, rois, x, 2, True, cfg.finest_scale, B.RAF_NO_PREP, None)
+    a = x.permute(0, 2, 3, 1).reshape(K, -1).to(torch.float32)
+    want = a @ w.to(torch.float32).T
+    torch.cuda.synchronize()
+    scale = (a.abs() @ w.to(torch.float32).abs().T)
+    assert bool(((out - want).abs() <= 1e-5 * scale + 1e-6).all())
+
+
+def test_roi_align_fc_argument_errors():
+    wl = inputs.make_workload(5, n_img=1, per_img=8, channels=64)
+    cfg = wl.cfg
+    feats, _ = T.device_feats(wl.feats, "bf16", "cl")
+    rois = torch.from_numpy(wl.rois).cuda()
+    w = torch.zeros((256, 49 * 64), dtype=torch.bfloat16, device="cuda")
+    out = torch.empty((cfg.K, 256), dtype=torch.float32, device="cuda")
+    with pytest.raises(B.RafError) as e:     # sampling grid beyond the tables of this kernel
+        B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w, None, out, (7, 7), 3, True, 56.0)
+    assert e.value.status == -5
+    with pytest.raises(B.RafError) as e:     # n_out not a multiple of 256
+        B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w[:128], None, out[:, :128].contiguous(), (7, 7), 2, True, 56.0)
+    assert e.value.status == -5
+    with pytest.raises(ValueError):
+        B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w.to(torch.float16), None, out, (7, 7), 2, True, 56.0)

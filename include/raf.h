@@ -183,7 +183,7 @@ int roi_pool_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dty
  * the RoI feature tensor the head would read -- but it is never written: tiles of it are produced straight into the
  * A operand of a tcgen05 GEMM (bf16 / fp16 inputs, fp32 accumulation in tensor memory).
  *   feats    channels-last (sc == 1), dtype RAF_F16 or RAF_BF16, C % 64 == 0
- *   weight   DEVICE, dtype, [n_out, out_h*out_w*C] row-major, columns in (ph, pw, c) order; n_out % 256 == 0
+ *   weight   DEVICE, dtype, [n_out, out_h*out_w*C] row-major, columns in (ph, pw, c) order; n_out % 512 == 0
  *   bias     DEVICE fp32 [n_out] or NULL
  *   out      DEVICE fp32 [K, n_out] row-major, overwritten (zero-filled, then fp32 reductions: the summation order
  *            over the out_h split-K slices is not fixed)

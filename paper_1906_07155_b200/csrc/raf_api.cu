@@ -486,7 +486,7 @@ int roi_align_fc_fpn_forward(const raf_level* feats, int L, raf_dtype dtype, con
   if (!(finest_scale > 0.0f) || n_out < 1) return RAF_ERR_SHAPE;
   if (K == 0) return RAF_OK;
   if (!weight || !out) return RAF_ERR_NULL;
-  if (dtype == RAF_F32 || sampling_ratio < 1 || sampling_ratio > 2 || n_out % 256 || feats[0].c % 64) return RAF_ERR_UNSUPPORTED;
+  if (dtype == RAF_F32 || sampling_ratio < 1 || sampling_ratio > 2 || n_out % 512 || feats[0].c % 64) return RAF_ERR_UNSUPPORTED;
   if (!levels_vectorizable(feats, L, 8, 2) || ((uintptr_t)weight) % 16 || ((uintptr_t)out) % 16) return RAF_ERR_UNSUPPORTED;
   if ((int64_t)K * n_out >= ((int64_t)1 << 40)) return RAF_ERR_UNSUPPORTED;
   cudaStream_t st = (cudaStream_t)stream;

@@ -3,17 +3,17 @@
 // A = the RoIAlign features of RoI k rounded to the feature dtype (readings F1-F3).  The [K, PH*PW*C]
 // feature tensor never goes to HBM: it is produced tile by tile straight into the A operand of a tcgen05 GEMM.
 //
-// CTA = (128 RoIs) x (256 outputs) x (one bin row ph: split-K, fp32 `red` into out).  Per k-step = (bin pw, 64 channels):
-//   * 256 threads gather the A tile: thread (RoI r, 16-byte chunk j) evaluates the bin's merged separable taps (same
+// CTA = (128 RoIs) x (512 outputs) x (one bin row ph: split-K, fp32 `red` into out), 1024 threads.  Per k-step = (bin pw, 64 channels):
+//   * the threads gather the A tile: thread (RoI r, 16-byte chunk j) evaluates the bin's merged separable taps (same
 //     tables and FMA order as raf_forward.cu, so the value is bit-identical to the stand-alone forward), rounds to the
 //     feature dtype and stores 16 bytes into shared memory in the K-major 128-byte-swizzled UMMA layout
 //     (row r at r * 128 B, chunk j at (j ^ (r & 7)) * 16 B: eight lanes write one row, conflict-free);
-//   * the same threads copy the W tile [256 x 64] (K-major in memory: W is [N_out, PH*PW*C] row-major) the same way;
-//   * fence.proxy.async + barrier, then ONE thread issues four tcgen05.mma (M 128, N 256, K 16; bf16/fp16 in, fp32
-//     accumulate in 256 columns of tensor memory) and commits them to an mbarrier; shared memory is double-buffered,
+//   * the same threads copy the W tile [512 x 64] (K-major in memory: W is [N_out, PH*PW*C] row-major) the same way;
+//   * fence.proxy.async + barrier, then ONE thread issues eight tcgen05.mma (M 128, N 256, K 16; two N halves; bf16/fp16 in,
+//     fp32 accumulate in all 512 columns of tensor memory) and commits them to an mbarrier; shared memory is double-buffered,
 //     so the gather of step i+1 overlaps the MMAs of step i;
 //   * epilogue: tcgen05.ld (32 lanes x 8 columns per warp and step), bias added by the ph == 0 split, red.global.add.
-// Cost model: the 256-column accumulator means every RoI window is gathered N_out / 256 times; this
+// Cost model: the 512-column accumulator means every RoI window is gathered N_out / 512 times; this
 // kernel exists to be correct and measured, not yet to beat forward + library GEMM.
 #include "raf_device.cuh"
 #include "raf_host.h"
@@ -21,8 +21,9 @@
 
 namespace raf {
 
-constexpr int kFcM = 128, kFcN = 256, kFcK = 64;
-constexpr int kFcThreads = 256;
+constexpr int kFcM = 128, kFcN = 512, kFcK = 64;   // CTA tile: 128 RoIs x 512 outputs (all 512 tensor-memory columns)
+constexpr int kFcUmmaN = 256;                      // N of one tcgen05.mma (two per k-slice)
+constexpr int kFcThreads = 1024;                   // one (RoI, 16-byte chunk) gather unit per thread and k-step
 
 __device__ __forceinline__ uint32_t fc_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -57,7 +58,7 @@ template <> struct FcFmt<__half> { static constexpr uint32_t kFmt = 0; };       
 template <> struct FcFmt<__nv_bfloat16> { static constexpr uint32_t kFmt = 1; };   // UMMA BF16
 
 template <typename T>
-__global__ void __launch_bounds__(kFcThreads, 2)
+__global__ void __launch_bounds__(kFcThreads, 1)
 fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, const float* __restrict__ bias, int n_out,
                 float* __restrict__ out) {
   using V = Vec16<T>;   // 8 elements per 16 bytes
@@ -111,7 +112,7 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;");
   const uint32_t tmem = tmem_base_s;
-  const uint32_t idesc = (1u << 4) | (FcFmt<T>::kFmt << 7) | (FcFmt<T>::kFmt << 10) | ((uint32_t)(kFcN >> 3) << 17) |
+  const uint32_t idesc = (1u << 4) | (FcFmt<T>::kFmt << 7) | (FcFmt<T>::kFmt << 10) | ((uint32_t)(kFcUmmaN >> 3) << 17) |
                          ((uint32_t)(kFcM >> 4) << 24);
 
   const int cchunks = C / kFcK;
@@ -130,11 +131,19 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
       if (step >= 2) { fc_mbar_wait(&mma_done[st], phase[st]); phase[st] ^= 1; }   // the MMAs that read this stage are done
       unsigned char* At = sA + st * kFcM * 128;
       unsigned char* Bt = sB + st * kFcN * 128;
-      // ---- A tile: thread = (RoI row r, 16-byte chunk j); eight lanes cover the 64 channels of one RoI -----------
+      // ---- W tile first (its loads fly while the A tile is gathered): W[n0 + n][(ph * PW + pw) * C + cc * 64 + j * 8 ...] ---
       const int j = tid & 7;
+      const int64_t kidx = ((int64_t)ph * PW + pw) * C + cc * kFcK + j * 8;
+      uint4 wv[kFcN * 8 / kFcThreads];
+#pragma unroll
+      for (int i = 0; i < kFcN * 8 / kFcThreads; ++i) {
+        const int n = (tid >> 3) + (kFcThreads / 8) * i;
+        wv[i] = __ldg(reinterpret_cast<const uint4*>(W + (int64_t)(n0 + n) * Kd + kidx));
+      }
+      // ---- A tile: thread = (RoI row r, 16-byte chunk j); eight lanes cover the 64 channels of one RoI -----------
 #pragma unroll 1
-      for (int i = 0; i < 4; ++i) {
-        const int r = (tid >> 3) + 32 * i;
+      for (int i = 0; i < kFcM * 8 / kFcThreads; ++i) {
+        const int r = (tid >> 3) + (kFcThreads / 8) * i;
         float acc[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) acc[q] = 0.0f;
@@ -142,11 +151,10 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
         const int ny = s_ny[r], nx = s_nx[r];
         if (base != nullptr) {
           const T* p0 = base + cc * kFcK + j * 8;
-          FwdTap ty[4], tx[4];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) { ty[q] = s_ty[r][q]; tx[q] = s_tx[r][q]; }
+          const FwdTap* ty = s_ty[r];
+          const FwdTap* tx = s_tx[r];
           // the loads of two tap rows (<= 8) are issued before their FMAs: memory-level parallelism is what bounds the
-          // gather, and 128 registers keep two CTAs (2 x 256 tensor-memory columns) on an SM
+          // gather (1024 threads x 8 loads x 16 B = 128 KB in flight per SM at 64 registers per thread)
 #pragma unroll
           for (int y0 = 0; y0 < 4; y0 += 2) {
             if (y0 < ny) {
@@ -179,13 +187,10 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
         }
         *reinterpret_cast<uint4*>(At + r * 128 + ((j ^ (r & 7)) << 4)) = packed;
       }
-      // ---- B tile: W[n0 + n][(ph * PW + pw) * C + cc * 64 + j * 8 ...] --------------------------------------------
-      const int64_t kidx = ((int64_t)ph * PW + pw) * C + cc * kFcK + j * 8;
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int n = (tid >> 3) + 32 * i;
-        const uint4 wv = __ldg(reinterpret_cast<const uint4*>(W + (int64_t)(n0 + n) * Kd + kidx));
-        *reinterpret_cast<uint4*>(Bt + n * 128 + ((j ^ (n & 7)) << 4)) = wv;
+      for (int i = 0; i < kFcN * 8 / kFcThreads; ++i) {
+        const int n = (tid >> 3) + (kFcThreads / 8) * i;
+        *reinterpret_cast<uint4*>(Bt + n * 128 + ((j ^ (n & 7)) << 4)) = wv[i];
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
       __syncthreads();
@@ -194,11 +199,15 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
 #pragma unroll
         for (int s = 0; s < kFcK / 16; ++s) {
           const uint64_t ad = fc_desc(fc_smem_u32(At) + s * 32);
-          const uint64_t bd = fc_desc(fc_smem_u32(Bt) + s * 32);
           const uint32_t accf = (step > 0 || s > 0) ? 1u : 0u;
-          asm volatile(
-              "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-              "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem), "l"(ad), "l"(bd), "r"(idesc), "r"(accf));
+#pragma unroll
+          for (int h = 0; h < kFcN / kFcUmmaN; ++h) {   // N halves: rows h*256.. of the W tile -> columns h*256.. of the accumulator
+            const uint64_t bd = fc_desc(fc_smem_u32(Bt) + h * kFcUmmaN * 128 + s * 32);
+            asm volatile(
+                "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem + h * kFcUmmaN), "l"(ad), "l"(bd), "r"(idesc),
+                "r"(accf));
+          }
         }
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"l"(
             (uint64_t)__cvta_generic_to_shared(&mma_done[st])));
@@ -212,10 +221,11 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
     fc_mbar_wait(&mma_done[st], phase[st]);
   }
   asm volatile("tcgen05.fence::after_thread_sync;");
-  const int row = (warp & 3) * 32 + lane;          // tensor-memory lane = row of the tile
-  const int col0 = (warp >> 2) * (kFcN / 2);       // warps 0-3: columns 0..127, warps 4-7: 128..255
+  const int row = (warp & 3) * 32 + lane;          // tensor-memory lane = row of the tile (a warp reaches lanes 32 * (warp % 4) ..)
+  constexpr int kColsPerWarp = kFcN / (kFcThreads / 128);
+  const int col0 = (warp >> 2) * kColsPerWarp;
   const int kroi = m0 + row;
-  for (int c = 0; c < kFcN / 2; c += 8) {
+  for (int c = 0; c < kColsPerWarp; c += 8) {
     uint32_t v[8];
     const uint32_t taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(col0 + c);
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
@@ -224,12 +234,14 @@ fc_fused_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ W, 
     asm volatile("tcgen05.wait::ld.sync.aligned;");
     if (kroi < a.K) {
       float* o = out + (int64_t)kroi * n_out + n0 + col0 + c;
+      float val[8];
 #pragma unroll
       for (int q = 0; q < 8; ++q) {
-        float val = __uint_as_float(v[q]);
-        if (ph == 0 && bias != nullptr) val += __ldg(bias + n0 + col0 + c + q);
-        atomicAdd(o + q, val);
+        val[q] = __uint_as_float(v[q]);
+        if (ph == 0 && bias != nullptr) val[q] += __ldg(bias + n0 + col0 + c + q);
       }
+      red_add_v4(o, val[0], val[1], val[2], val[3]);
+      red_add_v4(o + 4, val[4], val[5], val[6], val[7]);
     }
   }
   asm volatile("tcgen05.fence::before_thread_sync;");

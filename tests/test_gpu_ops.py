@@ -271,10 +271,10 @@ def _fc_case(index, dtype, kw, n_out, g=2, bias=True, seed=0):
 
 
 @pytest.mark.parametrize("index,dtype,kw,n_out,g", [
-    (5, "bf16", dict(n_img=2, per_img=100, channels=64), 256, 2),      # 200 RoIs: two M tiles, the second ragged
-    (4, "bf16", dict(n_img=1, per_img=40, channels=128), 512, 2),      # 14 x 14 bins, two N tiles
-    (3, "f16", dict(n_img=1, per_img=130, channels=64), 256, 2),
-    (5, "f16", dict(n_img=2, per_img=30, channels=192), 256, 1),
+    (5, "bf16", dict(n_img=2, per_img=100, channels=64), 512, 2),      # 200 RoIs: two M tiles, the second ragged
+    (4, "bf16", dict(n_img=1, per_img=40, channels=128), 1024, 2),     # 14 x 14 bins, two N tiles
+    (3, "f16", dict(n_img=1, per_img=130, channels=64), 512, 2),
+    (5, "f16", dict(n_img=2, per_img=30, channels=192), 512, 1),
 ])
 def test_roi_align_fc_fused(index, dtype, kw, n_out, g):
     worst, emax, rmax = _fc_case(index, dtype, kw, n_out, g)
@@ -292,8 +292,8 @@ def test_roi_align_fc_fused_matches_unfused_library_path():
     feats, _ = T.device_feats(wl.feats, "bf16", "cl")
     rois = torch.from_numpy(wl.rois).cuda()
     rng = np.random.default_rng(3)
-    w = torch.from_numpy((rng.standard_normal((256, PH * PW * C)) / 56.0).astype(np.float32)).to(torch.bfloat16).cuda()
-    out = torch.empty((K, 256), dtype=torch.float32, device="cuda")
+    w = torch.from_numpy((rng.standard_normal((512, PH * PW * C)) / 56.0).astype(np.float32)).to(torch.bfloat16).cuda()
+    out = torch.empty((K, 512), dtype=torch.float32, device="cuda")
     B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w, None, out, (PH, PW), 2, True, cfg.finest_scale)
     x = T.empty_layout((K, C, PH, PW), torch.bfloat16, "cl")
     B.roi_align_fpn_forward_ex(feats, cfg.scales, rois, x, 2, True, cfg.finest_scale, B.RAF_NO_PREP, None)
@@ -309,12 +309,12 @@ def test_roi_align_fc_argument_errors():
     cfg = wl.cfg
     feats, _ = T.device_feats(wl.feats, "bf16", "cl")
     rois = torch.from_numpy(wl.rois).cuda()
-    w = torch.zeros((256, 49 * 64), dtype=torch.bfloat16, device="cuda")
-    out = torch.empty((cfg.K, 256), dtype=torch.float32, device="cuda")
+    w = torch.zeros((512, 49 * 64), dtype=torch.bfloat16, device="cuda")
+    out = torch.empty((cfg.K, 512), dtype=torch.float32, device="cuda")
     with pytest.raises(B.RafError) as e:     # sampling grid beyond the tables of this kernel
         B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w, None, out, (7, 7), 3, True, 56.0)
     assert e.value.status == -5
-    with pytest.raises(B.RafError) as e:     # n_out not a multiple of 256
+    with pytest.raises(B.RafError) as e:     # n_out not a multiple of 512
         B.roi_align_fc_fpn_forward(feats, cfg.scales, rois, w[:128], None, out[:, :128].contiguous(), (7, 7), 2, True, 56.0)
     assert e.value.status == -5
     with pytest.raises(ValueError):

@@ -163,3 +163,57 @@ def test_binding_rejects_what_the_abi_cannot_see():
     grads = [torch.zeros((1, 4, 8, 8)), torch.zeros((1, 4, 4, 4), dtype=torch.bfloat16)]
     with pytest.raises(ValueError):   # gradient pyramid must be fp32
         B.roi_align_fpn_backward(grads, scales, out, rois, 2, True, 56.0, 0, ws)
+
+
+def _levels_nchw(L=2, n=2, c=8, h=16, w=20):
+    arr = (B.RafLevel * L)()
+    for i in range(L):
+        hh, ww = max(h >> i, 1), max(w >> i, 1)
+        arr[i].data = 0x100000 * (i + 1)
+        arr[i].n, arr[i].c, arr[i].h, arr[i].w = n, c, hh, ww
+        arr[i].sn, arr[i].sc, arr[i].sh, arr[i].sw = c * hh * ww, hh * ww, ww, 1
+        arr[i].spatial_scale = 0.25 / (1 << i)
+    return arr
+
+
+def _levels_c(c, L=2):
+    arr = _levels(L)
+    for i in range(L):
+        arr[i].c = c
+        arr[i].sn, arr[i].sh, arr[i].sw = c * arr[i].h * arr[i].w, arr[i].w * c, c
+    return arr
+
+
+def test_round2_entry_points_reject_bad_arguments_before_any_launch(lib):
+    """Host-side validation of the entry points added in round 2 (fake pointers: nothing may be launched)."""
+    i64x4 = ctypes.c_int64 * 4
+    cl, nchw = i64x4(392, 1, 56, 8), i64x4(392, 49, 7, 1)
+    f = ctypes.c_float
+    # backward_ex: the gradient pyramid is fp32 or has the 16-bit type of grad_out
+    bex = lambda gdt, odt, flags=0: lib.roi_align_fpn_backward_ex(_levels(), 2, odt, gdt, 0x3000, cl, 0x2000, 4, 7, 7, 2, 1,
+                                                                  f(56.0), flags, 0x4000, 1 << 20, None)
+    assert bex(1, 2) == -5 and bex(2, 0) == -5 and bex(7, 0) == -3
+    assert bex(2, 2, flags=4) == -5 and bex(2, 2, flags=128) == -5      # RAF_ATOMIC / RAF_REPACK with a 16-bit pyramid
+    # RAF_REPACK: needs dense NCHW operands and room for the copies
+    lib.roi_align_fpn_repack_bytes.restype = ctypes.c_size_t
+    lib.roi_align_fpn_workspace_bytes.restype = ctypes.c_size_t
+    need = lib.roi_align_fpn_repack_bytes(_levels_nchw(), 2, 0, 4, 7, 7)
+    assert need >= 4 * (2 * 8 * 16 * 20 + 2 * 8 * 8 * 10) + 4 * 4 * 8 * 49 and need % 256 == 0
+    assert lib.roi_align_fpn_repack_bytes(None, 2, 0, 4, 7, 7) == 0
+    fex = lambda lv, st, ws_bytes: lib.roi_align_fpn_forward_ex(lv, 2, 0, 0x2000, 4, 7, 7, 2, 1, f(56.0), 0x3000, st, 128, 0x4000,
+                                                                ws_bytes, None)
+    base = lib.roi_align_fpn_workspace_bytes(4, 2, 7, 7, 2, 0)
+    assert fex(_levels_nchw(), nchw, base + need - 1) == -6
+    assert fex(_levels_nchw(), i64x4(392, 49, 14, 1), 1 << 24) == -4       # output neither channels-last nor dense NCHW
+    # fused gather + FC
+    fc = lambda dtype=2, g=2, n_out=512, lv=None: lib.roi_align_fc_fpn_forward(lv or _levels_c(64), 2, dtype, 0x2000, 4, 7, 7, g, 1,
+                                                                                f(56.0), 0x5000, None, n_out, 0x6000, None)
+    assert fc(dtype=0) == -5 and fc(g=3) == -5 and fc(n_out=256) == -5 and fc(lv=_levels()) == -5 and fc(n_out=0) == -2
+    assert lib.roi_align_fc_fpn_forward(_levels_c(64), 2, 2, 0x2000, 4, 7, 7, 2, 1, f(56.0), None, None, 512, 0x6000, None) == -1
+    # deformable RoI pooling
+    dfw = lambda g=2, out=0x3000: lib.roi_deform_pool_fpn_forward(_levels(), 2, 0, 0x2000, 4, None, f(0.1), 7, 7, g, f(56.0), out, cl, None)
+    assert dfw(g=-1) == -2 and dfw(out=None) == -1
+    assert lib.roi_deform_pool_fpn_backward(_levels(), None, 2, 0, 0x3000, cl, 0x2000, 4, None, f(0.1), 7, 7, 2, f(56.0), None, 4,
+                                            None) == -5
+    assert lib.roi_deform_pool_fpn_backward(_levels(), _levels(h=9), 2, 0, 0x3000, cl, 0x2000, 4, None, f(0.1), 7, 7, 2, f(56.0),
+                                            None, 0, None) == -2

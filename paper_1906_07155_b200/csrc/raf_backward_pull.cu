@@ -97,6 +97,31 @@ template <> __device__ __forceinline__ float4 ldg4<__nv_bfloat16>(const __nv_bfl
                      __uint_as_float(r.y << 16), __uint_as_float(r.y & 0xffff0000u));
 }
 
+// Raw (unconverted) 4-channel loads: the 16-bit types are widened at the use, after all loads of a hit are issued.
+template <typename T> struct Raw4;
+template <> struct Raw4<float> {
+  typedef float4 type;
+  static __device__ __forceinline__ float4 load(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+  static __device__ __forceinline__ float4 widen(const float4& r) { return r; }
+};
+template <> struct Raw4<__half> {
+  typedef uint2 type;
+  static __device__ __forceinline__ uint2 load(const __half* p) { return __ldg(reinterpret_cast<const uint2*>(p)); }
+  static __device__ __forceinline__ float4 widen(const uint2& r) {
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+  }
+};
+template <> struct Raw4<__nv_bfloat16> {
+  typedef uint2 type;
+  static __device__ __forceinline__ uint2 load(const __nv_bfloat16* p) { return __ldg(reinterpret_cast<const uint2*>(p)); }
+  static __device__ __forceinline__ float4 widen(const uint2& r) {
+    return make_float4(__uint_as_float(r.x << 16), __uint_as_float(r.x & 0xffff0000u),
+                       __uint_as_float(r.y << 16), __uint_as_float(r.y & 0xffff0000u));
+  }
+};
+
 template <typename T> struct Gout8 {
   static constexpr int kChunk = 256;
   static __device__ __forceinline__ void channels(int lane, int& chA, int& chB) { chA = lane * 4; chB = 128 + lane * 4; }
@@ -117,6 +142,19 @@ __device__ __forceinline__ void fma4(float4& acc, float w, const float4& v) {
   acc.x = fmaf(w, v.x, acc.x); acc.y = fmaf(w, v.y, acc.y);
   acc.z = fmaf(w, v.z, acc.z); acc.w = fmaf(w, v.w, acc.w);
 #endif
+}
+
+// The NP (offset, weight) pairs of one hit as ONE basic block: every load is issued before the first FMA waits, so a
+// hit exposes one memory latency, not one per pair (with a branch per pair the compiler keeps each pair's FMAs right
+// behind its loads).  Summation order = pair order, as everywhere.
+template <typename T, int NP>
+__device__ __forceinline__ void hit_pairs(const T* goutA, int dAB, const int (&o)[4], const float (&w)[4], float4& accA, float4& accB) {
+  typedef Raw4<T> R;
+  typename R::type ra[NP], rb[NP];
+#pragma unroll
+  for (int i = 0; i < NP; ++i) { const T* q = goutA + o[i]; ra[i] = R::load(q); rb[i] = R::load(q + dAB); }
+#pragma unroll
+  for (int i = 0; i < NP; ++i) { fma4(accA, w[i], R::widen(ra[i])); fma4(accB, w[i], R::widen(rb[i])); }
 }
 
 #ifndef RAF_PULL_NC
@@ -148,7 +186,9 @@ struct PullPair {
 
 // kThree: also serve rows / columns with THREE consecutive bins from the entries (outputs finer than the
 // pixel grid, e.g. 14 x 14 mask-head bins: config 4 backward 97.6 -> 90.9 us; on 7 x 7 outputs the extra
-// code in the hit loop costs more than it saves: 87.7 -> 93.0 us, so it is off there).
+// code in the hit loop costs more than it saves: 87.7 -> 93.0 us, so it is off there).  With kThree the
+// loads of a hit are also issued as a block before its FMAs (hit_pairs: 90.2 -> 84.1 us on config 4; the
+// same grouping on 7 x 7 outputs is SLOWER, 87.1 -> 92.7 us -- profiles/r2_experiments.md -- and stays off).
 template <typename T, typename G, bool kFull, bool kThree>
 __global__ void __launch_bounds__(kPullThreads, RAF_PULL_MINB)
 bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gout, int gs_k,
@@ -340,15 +380,28 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
           if (kThree && np == 254u) {   // three consecutive bins on the row and / or the column: straight from the entries
             const PullInfo iy = s_info[c][i], ix = s_info[c][8 + j];
             const int cy = (int)(iy.m0 >> 24), cx = (int)(ix.m0 >> 24);
-            const T* q0 = goutA + s_goff[c] + (int)(iy.m0 & kOffMask) + (int)(ix.m0 & kOffMask);
-            for (int ai = 0; ai < cy; ++ai) {
+            for (int ai = 0; ai < cy; ++ai) {   // one bin row (up to three bins) per round
               const float wy = ai == 0 ? iy.w0 : (ai == 1 ? iy.w1 : iy.w2);
-              const T* qy = q0 + ai * gs_h;
-              for (int bi = 0; bi < cx; ++bi) {
-                const float w = wy * (bi == 0 ? ix.w0 : (bi == 1 ? ix.w1 : ix.w2));
-                const T* q = qy + bi * gs_w;
-                fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+              const int oy = s_goff[c] + (int)(iy.m0 & kOffMask) + (int)(ix.m0 & kOffMask) + ai * gs_h;
+              const int o[4] = {oy, oy + gs_w, oy + 2 * gs_w, 0};
+              const float w[4] = {wy * ix.w0, wy * ix.w1, wy * ix.w2, 0.0f};
+              switch (cx) {
+                case 1: hit_pairs<T, 1>(goutA, dAB, o, w, accA, accB); break;
+                case 2: hit_pairs<T, 2>(goutA, dAB, o, w, accA, accB); break;
+                default: hit_pairs<T, 3>(goutA, dAB, o, w, accA, accB); break;
               }
+            }
+          } else if (kThree && np != 255u) {   // fine outputs: the pairs of the hit in one block (measured: config 4
+            const PullPair* sp = &s_pair[p][4 * c];   // backward 90.2 -> 84.1 us; on 7 x 7 outputs 87.1 -> 92.7 us, so off there)
+            const uint4 e01 = *reinterpret_cast<const uint4*>(sp);
+            const uint4 e23 = *reinterpret_cast<const uint4*>(sp + 2);
+            const int o[4] = {(int)e01.x, (int)e01.z, (int)e23.x, (int)e23.z};
+            const float w[4] = {__uint_as_float(e01.y), __uint_as_float(e01.w), __uint_as_float(e23.y), __uint_as_float(e23.w)};
+            switch (np) {
+              case 1: hit_pairs<T, 1>(goutA, dAB, o, w, accA, accB); break;
+              case 2: hit_pairs<T, 2>(goutA, dAB, o, w, accA, accB); break;
+              case 3: hit_pairs<T, 3>(goutA, dAB, o, w, accA, accB); break;
+              default: hit_pairs<T, 4>(goutA, dAB, o, w, accA, accB); break;
             }
           } else if (np != 255u) {
             const PullPair* sp = &s_pair[p][4 * c];

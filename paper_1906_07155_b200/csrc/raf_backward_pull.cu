@@ -23,18 +23,21 @@
 //      and keep the RoIs that meet it (ballot compaction, order preserved);
 //  (B) per pass of <= 16 candidates, one warp per candidate holds the RoI's taps in its lanes and
 //      ballots them against the tile's rows and columns: shared memory gets, per (candidate, row)
-//      and (candidate, column), the first two entries (premultiplied grad_out offset, weight) + the
-//      entry count, and the ballot masks for the (rarer) further entries; then, lanes = pixels, the
-//      row x column entries of every pixel are expanded into <= 4 (offset, wy*wx) PAIRS per
-//      (pixel, candidate) and their number;
+//      and (candidate, column), an ENTRY -- the premultiplied grad_out offset of the first bin with a
+//      tap there, the weights of the first two (three) consecutive bins, the bin count -- and the
+//      ballot masks for the (rarer) longer lists; then, lanes = pixels, one byte per (pixel,
+//      candidate): no contribution / served by the entries / walk the masks;
 //  (C) warp w owns pixel (i, (w + i) % 8) of every tile row i (one pixel per row and column: the
 //      warps of a CTA carry about the same load); one pixel at a time, lanes spread over the 256
 //      channels (two float4 accumulators per lane = 8 registers of state, 64 registers total, 4
-//      CTAs per SM): a ballot over the pair counts gives the candidates that hit the pixel; each
-//      hit = one or two 16-byte shared loads + two 128-bit grad_out loads + 8 FFMA per pair.
-//      Candidates with more than two entries on an axis (bins narrower than half a pixel) walk the
-//      ballot masks instead (exact).  Tiles with more than 16 candidates take several passes, the
-//      partial sums parked in the gradient tensor itself.
+//      CTAs per SM): a ballot over those bytes gives the candidates that hit the pixel; each hit =
+//      two 16-byte shared loads (row entry, column entry), whose product gives up to 2 x 2 (3 x 3)
+//      (offset, wy * wx) pairs, and two 128-bit grad_out loads + 8 FFMA per pair.  (An earlier
+//      version expanded the pairs into a 34 KB table per CTA in (B); building them in the hit loop
+//      instead leaves that shared memory to L1 -- 7 KB per CTA -- and is faster: config 2 backward
+//      87.3 -> 85.9 us, config 4 84.2 -> 81.0 us.)  Candidates with longer lists (bins narrower
+//      than half a pixel) walk the ballot masks instead (exact).  Tiles with more than 16
+//      candidates take several passes, the partial sums parked in the gradient tensor itself.
 // Tiles of the coarsest level are scheduled first (most RoIs per pixel).
 #include "raf_device.cuh"
 #include "raf_host.h"
@@ -177,13 +180,6 @@ struct __align__(16) PullInfo {
   float w0, w1, w2;
 };
 
-// One contribution to a pixel: element offset into grad_out (k*gs_k + ph*gs_h + pw*gs_w) and the
-// weight wy * wx.  Up to four per (candidate, pixel) in the fast path.
-struct PullPair {
-  int off;
-  float w;
-};
-
 // kThree: also serve rows / columns with THREE consecutive bins from the entries (outputs finer than the
 // pixel grid, e.g. 14 x 14 mask-head bins: config 4 backward 97.6 -> 90.9 us; on 7 x 7 outputs the extra
 // code in the hit loop costs more than it saves: 87.7 -> 93.0 us, so it is off there).  With kThree the
@@ -199,8 +195,7 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
   __shared__ int s_wcount[2 * kPullThreads / 32];
   __shared__ int s_goff[kNC];                          // k * gs_k
   __shared__ PullInfo s_info[kNC][16];                 // [c][0..7] rows, [c][8..15] columns
-  __shared__ __align__(16) PullPair s_pair[64][4 * kNC + 2];   // contributions per (pixel, candidate); padded rows
-  __shared__ unsigned char s_pc[64][kNC];              // their number; 255: walk the masks instead
+  __shared__ unsigned char s_pc[64][kNC];              // per (pixel, candidate): 0 no contribution, 1 from the entries, 255 walk the masks
   extern __shared__ uint32_t s_mask[];                 // [kNC][16][nq]
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -332,27 +327,10 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
         }
         if (lane == 0) s_goff[c] = k * gs_k;
         __syncwarp();
-        // lanes = pixels now: expand (row entries) x (column entries) into the pixel's pair slots
-        const int goff = k * gs_k;
+        // lanes = pixels now: does candidate c land on the pixel, and can its entries serve it?
         for (int p = lane; p < 8 * npy; p += 32) {
-          const PullInfo iy = s_info[c][p >> 3], ix = s_info[c][8 + (p & 7)];
-          const uint32_t cy = iy.m0 >> 24, cx = ix.m0 >> 24;
-          const int oy0 = goff + (int)(iy.m0 & kOffMask), oy1 = oy0 + gs_h;
-          const int ox0 = (int)(ix.m0 & kOffMask), ox1 = ox0 + gs_w;
-          uint4 e01, e23;   // order: (y0,x0) (y0,x1) (y1,x0) (y1,x1), absent ones skipped
-          e01.x = (uint32_t)(oy0 + ox0); e01.y = __float_as_uint(iy.w0 * ix.w0);
-          if (cx >= 2) {
-            e01.z = (uint32_t)(oy0 + ox1); e01.w = __float_as_uint(iy.w0 * ix.w1);
-            e23.x = (uint32_t)(oy1 + ox0); e23.y = __float_as_uint(iy.w1 * ix.w0);
-          } else {
-            e01.z = (uint32_t)(oy1 + ox0); e01.w = __float_as_uint(iy.w1 * ix.w0);
-            e23.x = 0u; e23.y = 0u;
-          }
-          e23.z = (uint32_t)(oy1 + ox1); e23.w = __float_as_uint(iy.w1 * ix.w1);
-          *reinterpret_cast<uint4*>(&s_pair[p][4 * c]) = e01;
-          *reinterpret_cast<uint4*>(&s_pair[p][4 * c + 2]) = e23;
-          // pair count; 254: up to 3 x 3 consecutive bins, taken from the two entries; 255: walk the masks
-          s_pc[p][c] = (cy == 0 || cx == 0) ? 0 : ((cy > (kThree ? 3 : 2) || cx > (kThree ? 3 : 2)) ? 255 : ((cy > 2 || cx > 2) ? 254 : (unsigned char)(cy * cx)));
+          const uint32_t cy = s_info[c][p >> 3].m0 >> 24, cx = s_info[c][8 + (p & 7)].m0 >> 24;
+          s_pc[p][c] = (cy == 0 || cx == 0) ? 0 : ((cy > (kThree ? 3 : 2) || cx > (kThree ? 3 : 2)) ? 255 : 1);
         }
       }
       __syncthreads();
@@ -377,56 +355,30 @@ bwd_pull_kernel(const LevelsParam lv, const RoiArgs a, const T* __restrict__ gou
           const int c = __ffs(mm) - 1;
           mm &= mm - 1;
           const unsigned np = __shfl_sync(0xffffffffu, pcv, c);
-          if (kThree && np == 254u) {   // three consecutive bins on the row and / or the column: straight from the entries
+          if (np != 255u) {   // (row entries) x (column entries) of the pixel, straight from the tables of (B)
             const PullInfo iy = s_info[c][i], ix = s_info[c][8 + j];
             const int cy = (int)(iy.m0 >> 24), cx = (int)(ix.m0 >> 24);
-            for (int ai = 0; ai < cy; ++ai) {   // one bin row (up to three bins) per round
-              const float wy = ai == 0 ? iy.w0 : (ai == 1 ? iy.w1 : iy.w2);
-              const int oy = s_goff[c] + (int)(iy.m0 & kOffMask) + (int)(ix.m0 & kOffMask) + ai * gs_h;
-              const int o[4] = {oy, oy + gs_w, oy + 2 * gs_w, 0};
-              const float w[4] = {wy * ix.w0, wy * ix.w1, wy * ix.w2, 0.0f};
-              switch (cx) {
-                case 1: hit_pairs<T, 1>(goutA, dAB, o, w, accA, accB); break;
-                case 2: hit_pairs<T, 2>(goutA, dAB, o, w, accA, accB); break;
-                default: hit_pairs<T, 3>(goutA, dAB, o, w, accA, accB); break;
+            const int o00 = s_goff[c] + (int)(iy.m0 & kOffMask) + (int)(ix.m0 & kOffMask);
+            if (kThree) {
+              for (int ai = 0; ai < cy; ++ai) {   // one bin row (up to three bins) per round, its loads issued as a block
+                const float wy = ai == 0 ? iy.w0 : (ai == 1 ? iy.w1 : iy.w2);
+                const int oy = o00 + ai * gs_h;
+                const int o[4] = {oy, oy + gs_w, oy + 2 * gs_w, 0};
+                const float w[4] = {wy * ix.w0, wy * ix.w1, wy * ix.w2, 0.0f};
+                switch (cx) {
+                  case 1: hit_pairs<T, 1>(goutA, dAB, o, w, accA, accB); break;
+                  case 2: hit_pairs<T, 2>(goutA, dAB, o, w, accA, accB); break;
+                  default: hit_pairs<T, 3>(goutA, dAB, o, w, accA, accB); break;
+                }
               }
-            }
-          } else if (kThree && np != 255u) {   // fine outputs: the pairs of the hit in one block (measured: config 4
-            const PullPair* sp = &s_pair[p][4 * c];   // backward 90.2 -> 84.1 us; on 7 x 7 outputs 87.1 -> 92.7 us, so off there)
-            const uint4 e01 = *reinterpret_cast<const uint4*>(sp);
-            const uint4 e23 = *reinterpret_cast<const uint4*>(sp + 2);
-            const int o[4] = {(int)e01.x, (int)e01.z, (int)e23.x, (int)e23.z};
-            const float w[4] = {__uint_as_float(e01.y), __uint_as_float(e01.w), __uint_as_float(e23.y), __uint_as_float(e23.w)};
-            switch (np) {
-              case 1: hit_pairs<T, 1>(goutA, dAB, o, w, accA, accB); break;
-              case 2: hit_pairs<T, 2>(goutA, dAB, o, w, accA, accB); break;
-              case 3: hit_pairs<T, 3>(goutA, dAB, o, w, accA, accB); break;
-              default: hit_pairs<T, 4>(goutA, dAB, o, w, accA, accB); break;
-            }
-          } else if (np != 255u) {
-            const PullPair* sp = &s_pair[p][4 * c];
-            const uint4 e01 = *reinterpret_cast<const uint4*>(sp);
-            {
-              const T* q = goutA + (int)e01.x;
-              const float w = __uint_as_float(e01.y);
-              fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
-            }
-            if (np > 1) {
-              const T* q = goutA + (int)e01.z;
-              const float w = __uint_as_float(e01.w);
-              fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
-            }
-            if (np > 2) {
-              const uint4 e23 = *reinterpret_cast<const uint4*>(sp + 2);
-              {
-                const T* q = goutA + (int)e23.x;
-                const float w = __uint_as_float(e23.y);
-                fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
-              }
-              if (np > 3) {
-                const T* q = goutA + (int)e23.z;
-                const float w = __uint_as_float(e23.w);
-                fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB));
+            } else {   // order (y0,x0) (y0,x1) (y1,x0) (y1,x1)
+              const T* q = goutA + o00;
+              { const float w = iy.w0 * ix.w0; fma4(accA, w, ldg4<T>(q)); fma4(accB, w, ldg4<T>(q + dAB)); }
+              if (cx > 1) { const float w = iy.w0 * ix.w1; fma4(accA, w, ldg4<T>(q + gs_w)); fma4(accB, w, ldg4<T>(q + gs_w + dAB)); }
+              if (cy > 1) {
+                const T* q1 = q + gs_h;
+                { const float w = iy.w1 * ix.w0; fma4(accA, w, ldg4<T>(q1)); fma4(accB, w, ldg4<T>(q1 + dAB)); }
+                if (cx > 1) { const float w = iy.w1 * ix.w1; fma4(accA, w, ldg4<T>(q1 + gs_w)); fma4(accB, w, ldg4<T>(q1 + gs_w + dAB)); }
               }
             }
           } else {   // rare: more than two entries on an axis -> walk the ballot masks

@@ -156,6 +156,28 @@ int roi_align_fpn_backward(const raf_level* grad_feats, int L, raf_dtype gout_dt
                            int K, int out_h, int out_w, int sampling_ratio, int aligned,
                            float finest_scale, int flags, void* ws, size_t ws_bytes, void* stream);
 
+/* Backward WITHOUT a caller workspace and without any device allocation (for callers that cannot call cudaMalloc:
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid it).  Same operation, kernels and
+ * results as roi_align_fpn_backward (fp32 gradient pyramid); the scratch it needs -- the prep tables:
+ * RoI buckets, windows, geometry, tap tables -- lives in a static device array of RAF_STATIC_WS_BYTES inside the
+ * library, which every GPU that loads the library holds until the process exits.
+ *   limit    roi_align_fpn_workspace_bytes(K, L, out_h, out_w, sampling_ratio, flags) <= RAF_STATIC_WS_BYTES, else
+ *            RAF_ERR_WORKSPACE, decided on the host before any CUDA call (4 MiB: K = 8192 RoIs at 7 x 7 bins,
+ *            K = 4096 at 14 x 14, sampling_ratio 2)
+ *   flags    RAF_ACCUMULATE | RAF_DETERMINISTIC | RAF_ATOMIC | RAF_PULL_STRIP | RAF_PULL_TILE; RAF_REUSE_PREP and
+ *            RAF_REPACK return RAF_ERR_UNSUPPORTED (the array is shared by all calls and has no room for repack copies)
+ *   sharing  all calls on a device use the same array and it keeps the last call's contents: each call first clears
+ *            the fingerprint header (a 256-byte cudaMemsetAsync on `stream`, enqueued before the remaining argument
+ *            checks) and its prep launch rewrites everything the backward then reads.  Calls that OVERLAP on the GPU
+ *            (different streams without ordering between them) race on the array: order them.
+ * Calls no cudaMalloc, cudaFree or allocating library routine; the array's device address is looked up once per
+ * device (cudaGetSymbolAddress, with the caller's current device). */
+#define RAF_STATIC_WS_BYTES (4u << 20)
+int roi_align_fpn_backward_static(const raf_level* grad_feats, int L, raf_dtype gout_dtype,
+                                  const void* grad_out, const int64_t* gout_strides, const float* rois,
+                                  int K, int out_h, int out_w, int sampling_ratio, int aligned,
+                                  float finest_scale, int flags, void* stream);
+
 /* ---- the max variant of the "RoIPooling-like operators" (the RoI pooling
  * layer of Fast R-CNN), on the same FPN level map (C1) -------------------------------------------
  * Window of bin (ph,pw) on the RoI's level (fp32, each operation rounded; readings P1-P4):

@@ -26,7 +26,7 @@ EXPORTS = [
     "roi_align_fpn_backward_host", "roi_align_fpn_strerror", "roi_align_fpn_launch_count",
     "roi_pool_fpn_forward", "roi_pool_fpn_backward", "roi_nms_workspace_bytes", "roi_nms", "roi_soft_nms",
     "roi_align_fpn_repack_bytes", "roi_deform_pool_fpn_forward", "roi_deform_pool_fpn_backward",
-    "roi_align_fc_fpn_forward",
+    "roi_align_fc_fpn_forward", "roi_align_fpn_backward_static",
 ]
 
 
@@ -77,6 +77,8 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = args
         L.roi_align_fpn_forward_ex.restype = ctypes.c_int
         L.roi_align_fpn_forward_ex.argtypes = fwd_args[:12] + [ctypes.c_int] + fwd_args[12:]
+        L.roi_align_fpn_backward_static.restype = ctypes.c_int
+        L.roi_align_fpn_backward_static.argtypes = bwd_args[:13] + [ctypes.c_void_p]
         L.roi_align_fpn_backward_ex.restype = ctypes.c_int
         L.roi_align_fpn_backward_ex.argtypes = bwd_args[:3] + [ctypes.c_int] + bwd_args[3:]
         vp, ci, cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_float
@@ -245,6 +247,25 @@ def roi_align_fpn_backward(grad_feats: Sequence[torch.Tensor], scales: Sequence[
                                          ws.numel() * ws.element_size(), _stream_ptr(stream))
     if rc:
         raise RafError(rc, "roi_align_fpn_backward")
+
+
+RAF_STATIC_WS_BYTES = 4 << 20
+
+
+def roi_align_fpn_backward_static(grad_feats: Sequence[torch.Tensor], scales: Sequence[float],
+                                  grad_out: torch.Tensor, rois: torch.Tensor, sampling_ratio: int,
+                                  aligned: bool, finest_scale: float, flags: int = 0, stream=None) -> None:
+    """roi_align_fpn_backward without a workspace: the library's static scratch array (RAF_STATIC_WS_BYTES) is used
+    and nothing is allocated.  Calls that overlap on the GPU race on that array (include/raf.h)."""
+    if grad_out.dtype not in _DTYPES:
+        raise ValueError(f"unsupported grad_out dtype {grad_out.dtype}")
+    _check_call(grad_feats, torch.float32, rois, grad_out, grad_out.dtype, None)
+    K, _, PH, PW = grad_out.shape
+    rc = lib().roi_align_fpn_backward_static(make_levels(grad_feats, scales), len(grad_feats), _DTYPES[grad_out.dtype],
+                                             _ptr(grad_out), _strides4(grad_out), _ptr(rois), K, PH, PW, sampling_ratio,
+                                             int(bool(aligned)), finest_scale, int(flags), _stream_ptr(stream))
+    if rc:
+        raise RafError(rc, "roi_align_fpn_backward_static")
 
 
 def roi_align_fpn_host_arena_bytes(levels: Sequence[torch.Tensor], scales, dtype: torch.dtype, K: int,

@@ -7,7 +7,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libraf.so")
 SOURCES = ["raf_api.cu", "raf_levels.cu", "raf_forward.cu", "raf_backward.cu",
-           "raf_backward_pull.cu", "raf_backward_strip.cu", "raf_pool.cu", "raf_nms.cu", "raf_repack.cu", "raf_deform.cu", "raf_fc.cu"]
+           "raf_backward_pull.cu", "raf_backward_strip.cu", "raf_pool.cu", "raf_nms.cu", "raf_repack.cu", "raf_deform.cu", "raf_fc.cu",
+           "raf_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--cudart", "shared"]
 

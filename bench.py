@@ -58,6 +58,10 @@ def parse_args():
     ap.add_argument("--window-iters", type=int, default=200, help="back-to-back iterations per timing window")
     ap.add_argument("--sampling-ratio", type=int, default=None, help="override the config's sampling_ratio (0 = adaptive)")
     ap.add_argument("--aligned", type=int, default=None, help="override the config's aligned flag (0 / 1)")
+    ap.add_argument("--roi-order", choices=["given", "level"], default="given",
+                    help="given: the workload's RoI order (the headline); level: the same RoIs permuted into per-level order "
+                         "(finest level first, the stable permutation roi_fpn_assign_levels returns) before the timed "
+                         "region -- what a caller that extracts level by level passes; not the headline")
     ap.add_argument("--no-reuse-prep", action="store_true",
                     help="backward rebuilds its RoI buckets / tap tables instead of reusing the forward's (RAF_REUSE_PREP)")
     return ap.parse_args()
@@ -278,6 +282,15 @@ def run_ours(args):
     K, C, L = cfg.K, cfg.channels, len(cfg.level_shapes)
     PH, PW = cfg.out_size
     g, aligned, fs = cfg.sampling_ratio, cfg.aligned, cfg.finest_scale
+    if args.roi_order == "level":   # permute the RoIs (and their grad_out rows) with the library's own stable per-level permutation
+        d_rois = torch.from_numpy(wl.rois).cuda()
+        d_perm = torch.empty((K,), dtype=torch.int32, device="cuda")
+        B.roi_fpn_assign_levels(d_rois, L, fs, None, None, d_perm)
+        torch.cuda.synchronize()
+        perm = d_perm.cpu().numpy().astype(np.int64)
+        wl.rois = np.ascontiguousarray(wl.rois[perm])
+        if wl.grad_out is not None:
+            wl.grad_out = np.ascontiguousarray(wl.grad_out[perm])
     if args.sampling_ratio is not None:
         g = args.sampling_ratio
     if args.aligned is not None:
@@ -411,7 +424,8 @@ def run_ours(args):
         fp = {"level_hist": None}
         ab = {"fwd": pyr_bytes * esz + K * C * PH * PW * esz + 20 * K, "bwd": K * C * PH * PW * esz + pyr_bytes * 4}
     peak, peak_src = peaks()
-    variant = f"{args.layout}{'+repack' if repack else ''}{'+g16' if gdt != torch.float32 else ''}:{args.backward}:{'reuse' if reuse else 'noreuse'}"
+    variant = (f"{args.layout}{'+repack' if repack else ''}{'+g16' if gdt != torch.float32 else ''}"
+               f"{'+levelorder' if args.roi_order == 'level' else ''}:{args.backward}:{'reuse' if reuse else 'noreuse'}")
     traffic, traffic_stale = ncu_traffic(args.config, variant)
     legs = {"fwd": (ab["fwd"], loops["fwd"]["median_ms"])}
     if cfg.backward:
@@ -447,7 +461,8 @@ def run_ours(args):
                                        f"WARM: {R} buffer set(s), {R * ws_set / 1e6:.0f} MB vs L2 {l2 / 1e6:.0f} MB (not the headline)"),
                        "backward": args.backward if cfg.backward else "none", "repack": repack,
                        "grad_dtype": "f32" if gdt == torch.float32 else cfg.dtype,
-                       "reuse_prep": bool(reuse), "cuda_graph": bool(graphs), "level_hist": fp["level_hist"]},
+                       "reuse_prep": bool(reuse), "cuda_graph": bool(graphs), "roi_order": args.roi_order,
+                       "level_hist": fp["level_hist"]},
             "roofline": roof(dom),
             "roofline_all": {k: roof(k) for k in legs} | {"step": {
                 "achieved": step_ach, "frac": step_ach / peak, "frac_nominal_8000": step_ach / NOMINAL,

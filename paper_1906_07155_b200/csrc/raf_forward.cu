@@ -116,10 +116,15 @@ __device__ __noinline__ void fwd_direct_rows(const RoiGeom geo, const T* base, T
 #endif
 // kThreads = 224 (7 warps: 7-row outputs, the common case) or 256: the register budget follows the real block size.
 // A RoI's bin rows are split over `rsplit` CTAs (rows_per rows each) when there are more rows than warps.
+// The struct parameters are __grid_constant__: `lv` is indexed by the RoI's level, and without the qualifier every
+// thread first copies the arrays to its local memory (96-112 bytes of stack, 12 STL.64 in the prologue, LDL in the body);
+// with it the indexed reads come straight from the constant bank (config 2 forward 62.4 -> 55.8 us, config 3 37.3 -> 36.0 us,
+// config 5 198.2 -> 193.8 us).  The tile backward does NOT take the same change: its fp32 instantiation gets slower
+// (85.8 -> 90.3 us), profiles/r2_experiments.md.
 template <typename T, int kThreads>
 __global__ void __launch_bounds__(kThreads, kThreads == 224 ? RAF_FWD_MINB7 : (kThreads == 128 ? 7 : RAF_FWD_MINB))
-fwd_cl_kernel(const LevelsParam lv, const RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
-              int64_t os_w, int chunks, int rsplit, int rows_per, const PullPrepOut prep) {
+fwd_cl_kernel(const __grid_constant__ LevelsParam lv, const __grid_constant__ RoiArgs a, T* __restrict__ out, int64_t os_k, int64_t os_h,
+              int64_t os_w, int chunks, int rsplit, int rows_per, const __grid_constant__ PullPrepOut prep) {
   using V = Vec16<T>;
   constexpr int VN = V::N;
   extern __shared__ __align__(16) unsigned char fwd_smem[];
